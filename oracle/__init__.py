@@ -1,0 +1,176 @@
+"""ctypes front end of the CPU oracle (oracle/xodiac_oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this.  It imports nothing from the CUDA package; it takes any object with the
+network attributes (composition, nasa_lo, ..., t_ref) as plain numpy arrays.
+
+`Oracle()` loads the long-double build (parity checks); `Oracle(extended=False)` loads the
+pure-fp64 build (the one timed as the CPU baseline).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "xodiac_oracle.c")
+_LIBS = {True: os.path.join(_HERE, "liboracle.so"), False: os.path.join(_HERE, "liboracle_f64.so")}
+
+
+def build(force=False):
+    """Compile both oracle builds with gcc -O2 (no fast-math)."""
+    for extended, out in _LIBS.items():
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+            continue
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-o", out, _SRC, "-lm"]
+        if not extended:
+            cmd.insert(1, "-DXOD_ORACLE_DOUBLE")
+        subprocess.run(cmd, check=True)
+
+
+class _Net(C.Structure):
+    _fields_ = [("n_species", C.c_int), ("n_elements", C.c_int), ("n_reactions", C.c_int),
+                ("composition", C.c_void_p), ("nasa_lo", C.c_void_p), ("nasa_hi", C.c_void_p),
+                ("t_mid", C.c_void_p), ("type", C.c_void_p), ("reactants", C.c_void_p),
+                ("products", C.c_void_p), ("reversible", C.c_void_p), ("arrh", C.c_void_p),
+                ("arrh_low", C.c_void_p), ("troe_fc", C.c_void_p), ("t_ref", C.c_void_p)]
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p) if a is not None else None
+
+
+class Oracle:
+    def __init__(self, extended=True):
+        build()
+        self.lib = C.CDLL(_LIBS[bool(extended)])
+        self.extended = bool(extended)
+        L = self.lib
+        L.orc_real_mant_dig.restype = C.c_int
+        for name in ("orc_source_csr", "orc_jac_pattern", "orc_jacobian"):
+            getattr(L, name).restype = C.c_long
+        self.mant_dig = L.orc_real_mant_dig()
+
+    # -- network marshalling (keeps the numpy arrays alive next to the struct)
+    def _net(self, net):
+        keep = {
+            "composition": np.ascontiguousarray(net.composition, dtype=np.int32),
+            "nasa_lo": _f64(net.nasa_lo), "nasa_hi": _f64(net.nasa_hi), "t_mid": _f64(net.t_mid),
+            "type": np.ascontiguousarray(net.type, dtype=np.int32),
+            "reactants": np.ascontiguousarray(net.reactants, dtype=np.int32),
+            "products": np.ascontiguousarray(net.products, dtype=np.int32),
+            "reversible": np.ascontiguousarray(net.reversible, dtype=np.uint8),
+            "arrh": _f64(net.arrh), "arrh_low": _f64(net.arrh_low), "troe_fc": _f64(net.troe_fc),
+            "t_ref": None if getattr(net, "t_ref", None) is None else _f64(net.t_ref),
+        }
+        ns, ne = keep["composition"].shape
+        s = _Net(ns, ne, keep["type"].shape[0], *[_ptr(keep[k]) for k in (
+            "composition", "nasa_lo", "nasa_hi", "t_mid", "type", "reactants", "products",
+            "reversible", "arrh", "arrh_low", "troe_fc", "t_ref")])
+        return s, keep
+
+    @staticmethod
+    def _dims(net):
+        return int(np.shape(net.composition)[0]), int(np.shape(net.type)[0])
+
+    def thermo(self, net, T, ncol=None):
+        """cp/R, H/RT, S/R, G/RT, each [n_species][ld]."""
+        T = _f64(T)
+        ld = T.shape[0]
+        ncol = ld if ncol is None else ncol
+        ns, _ = self._dims(net)
+        s, keep = self._net(net)
+        out = [np.zeros((ns, ld)) for _ in range(4)]
+        self.lib.orc_thermo(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(T), *[_ptr(o) for o in out])
+        return tuple(out)
+
+    def rate_coeffs(self, net, T, P, J, ncol=None):
+        """k_f, k_r [n_reactions][ld] in user reaction order."""
+        T, P = _f64(T), _f64(P)
+        ld = T.shape[0]
+        ncol = ld if ncol is None else ncol
+        _, nr = self._dims(net)
+        J = _f64(J).reshape(-1, ld) if J is not None and np.size(J) else np.zeros((0, ld))
+        s, keep = self._net(net)
+        kf, kr = np.zeros((nr, ld)), np.zeros((nr, ld))
+        self.lib.orc_rate_coeffs(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(T), _ptr(P), _ptr(J),
+                                 _ptr(kf), _ptr(kr))
+        return kf, kr
+
+    def rates(self, net, kf, kr, n, ncol=None):
+        kf, kr, n = _f64(kf), _f64(kr), _f64(n)
+        ld = n.shape[1]
+        ncol = ld if ncol is None else ncol
+        s, keep = self._net(net)
+        qf, qr = np.zeros_like(kf), np.zeros_like(kr)
+        self.lib.orc_rates(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(kf), _ptr(kr), _ptr(n),
+                           _ptr(qf), _ptr(qr))
+        return qf, qr
+
+    def source(self, net, kf, kr, n, ncol=None):
+        """dn/dt, P, L [n_species][ld]."""
+        kf, kr, n = _f64(kf), _f64(kr), _f64(n)
+        ld = n.shape[1]
+        ncol = ld if ncol is None else ncol
+        s, keep = self._net(net)
+        out = [np.zeros_like(n) for _ in range(3)]
+        rc = self.lib.orc_source(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(kf), _ptr(kr), _ptr(n),
+                                 *[_ptr(o) for o in out])
+        assert rc == 0
+        return tuple(out)
+
+    def source_from_state(self, net, T, P, J, n, ncol=None):
+        """The whole path a1..a8: (T, P, J, n) -> dn/dt, P, L (k_f, k_r rounded to double between)."""
+        kf, kr = self.rate_coeffs(net, T, P, J, ncol)
+        return self.source(net, kf, kr, n, ncol)
+
+    def source_csr(self, net):
+        ns, _ = self._dims(net)
+        s, keep = self._net(net)
+        row_ptr = np.zeros(ns + 1, dtype=np.int64)
+        nnz = self.lib.orc_source_csr(C.byref(s), _ptr(row_ptr), None, None)
+        rxn, nu = np.zeros(nnz, dtype=np.int32), np.zeros(nnz, dtype=np.int32)
+        self.lib.orc_source_csr(C.byref(s), _ptr(row_ptr), _ptr(rxn), _ptr(nu))
+        return row_ptr, rxn, nu
+
+    def jac_pattern(self, net):
+        ns, _ = self._dims(net)
+        s, keep = self._net(net)
+        row_ptr = np.zeros(ns + 1, dtype=np.int64)
+        nnz = self.lib.orc_jac_pattern(C.byref(s), _ptr(row_ptr), None)
+        col = np.zeros(nnz, dtype=np.int32)
+        self.lib.orc_jac_pattern(C.byref(s), _ptr(row_ptr), _ptr(col))
+        return row_ptr, col
+
+    def jacobian_dense(self, net, kf, kr, n, c):
+        """Dense [n_species][n_species] Jacobian and tolerance scale of column c."""
+        kf, kr, n = _f64(kf), _f64(kr), _f64(n)
+        ns, _ = self._dims(net)
+        s, keep = self._net(net)
+        d, sc = np.zeros((ns, ns)), np.zeros((ns, ns))
+        rc = self.lib.orc_jacobian_dense(C.byref(s), C.c_long(n.shape[1]), _ptr(kf), _ptr(kr), _ptr(n),
+                                         C.c_long(c), _ptr(d), _ptr(sc))
+        assert rc == 0
+        return d, sc
+
+    def jacobian(self, net, kf, kr, n, row_ptr, col, ncol=None):
+        """Pattern values and scales [nnz][ld]; asserts the dense matrix is zero off-pattern."""
+        kf, kr, n = _f64(kf), _f64(kr), _f64(n)
+        ld = n.shape[1]
+        ncol = ld if ncol is None else ncol
+        s, keep = self._net(net)
+        row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)
+        col = np.ascontiguousarray(col, dtype=np.int32)
+        jac, sc = np.zeros((col.shape[0], ld)), np.zeros((col.shape[0], ld))
+        bad = self.lib.orc_jacobian(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(kf), _ptr(kr),
+                                    _ptr(n), _ptr(row_ptr), _ptr(col), _ptr(jac), _ptr(sc))
+        if bad != 0:
+            raise AssertionError("oracle: %d dense Jacobian entries outside the pattern are non-zero" % bad)
+        return jac, sc

@@ -1,0 +1,423 @@
+/* xodiac_oracle.c -- CPU ORACLE for the XODIAC chemical source term.  TEST INFRASTRUCTURE ONLY.
+ *
+ * A plain, slow, single-threaded, obviously-correct evaluation of what the hot path
+ * computes, written from the paper (arxiv 2512.06729, /root/reference/PAPER.md) and the
+ * readings listed in DESIGN.md.  It shares no code, header, table or helper with the CUDA
+ * library: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+ * reference legs may load it.  The product path never calls it.
+ *
+ * Method = direct evaluation of closed-form definitions, so the oracle is those
+ * definitions written out, one column at a time, with direct powl/expl/log10l calls:
+ * no log-domain folding, no type sorting, no precomputed per-reaction coefficients, no
+ * blocking, no sparse tricks (the Jacobian is filled as a dense N_s x N_s matrix and the
+ * pattern entries are read out of it).
+ *
+ * Precision: inputs and outputs are IEEE double (the path's arithmetic type).  Internal
+ * values are `real_t` = long double (x86-64 80-bit extended) so that (i) the oracle's own
+ * rounding error is far below the 1e-12 parity tolerance and (ii) K_c = exp(-dG/RT) never
+ * overflows before k_r = k_f / K_c is rounded to double (reading R5).  Building
+ * with -DXOD_ORACLE_DOUBLE makes real_t = double: the pure-fp64 variant that is timed as
+ * the CPU baseline and cross-checked against the extended one in tests.
+ *
+ * Units: cgs.  T [K], P [dyn cm^-2], n [cm^-3], k [s^-1, cm^3 s^-1, cm^6 s^-1], J [s^-1].
+ * Layout: every per-column array is [row][ld], column index contiguous, ld >= ncol.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Table 1 coefficients against textbook
+ * thermochemistry of H2O, CO2 and a monatomic gas, G = H - TS, calculus
+ * identities between cp, H and S, the n = 0, E = 0 => k = A case, Lindemann limits, Troe
+ * symmetry, K_c recomputed from the thermo outputs by the test, element conservation, the
+ * equilibrium fixed point, hand-expanded rate laws on a 3-species network, finite
+ * differences of dn/dt against the Jacobian, and brute-force CSR construction.
+ * Nothing here is "parity unpinned".
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef XOD_ORACLE_DOUBLE
+typedef double real_t;
+#define R_EXP exp
+#define R_LOG log
+#define R_LOG10 log10
+#define R_POW pow
+#define R_FABS fabs
+#else
+typedef long double real_t;
+#define R_EXP expl
+#define R_LOG logl
+#define R_LOG10 log10l
+#define R_POW powl
+#define R_FABS fabsl
+#endif
+
+/* physical constants (cgs); BASELINE.json north_star: [M] = P/(k_B T); T2: P0 = 1 bar */
+static const real_t K_BOLTZ = (real_t)1.380649e-16L; /* erg/K, exact SI 2019 value */
+static const real_t P_REF = (real_t)1.0e6L;          /* dyn/cm^2 = 1 bar */
+
+enum { ORC_UNI = 0, ORC_BI = 1, ORC_FALLOFF = 2, ORC_PHOTO = 3 };
+
+/* The reaction record of PAPER.md:105-157: type, reactants, products, Arrhenius/Kooij
+ * constants (alpha, beta, gamma) and, for three-body reactions, the low-pressure set. */
+typedef struct {
+  int n_species, n_elements, n_reactions;
+  const int *composition;          /* [n_species][n_elements] */
+  const double *nasa_lo, *nasa_hi; /* [n_species][7]  a1..a7 */
+  const double *t_mid;             /* [n_species] */
+  const int *type;                 /* [n_reactions] */
+  const int *reactants, *products; /* [n_reactions][3], -1 padded, repeated index = coefficient 2 */
+  const unsigned char *reversible; /* [n_reactions] */
+  const double *arrh;              /* [n_reactions][3] alpha, beta, gamma   (k_inf for FALLOFF) */
+  const double *arrh_low;          /* [n_reactions][3] alpha0, beta0, gamma0 (FALLOFF only) */
+  const double *troe_fc;           /* [n_reactions] */
+  const double *t_ref;             /* [n_reactions] 1 = modified Arrhenius, 300 = Kooij; NULL -> 1 */
+} orc_network;
+
+int orc_real_bits(void) { return (int)(sizeof(real_t) * 8); }
+int orc_real_mant_dig(void) {
+#ifdef XOD_ORACLE_DOUBLE
+  return 53;
+#else
+  return __LDBL_MANT_DIG__;
+#endif
+}
+
+/* ---------------------------------------------------------------- O1 thermo (NASA-7)
+ * two coefficient sets, low- and high-temperature range.
+ * PAPER.md:671  G/RT = a1(1 - ln T) - a2 T/2 - a3 T^2/6 - a4 T^3/12 - a5 T^4/20 + a6/T - a7
+ * PAPER.md:673  cp/R = a1 + a2 T + a3 T^2 + a4 T^3 + a5 T^4
+ * H/RT and S/R are not printed; the standard NASA-7 forms are used (reading T1):
+ *   H/RT = a1 + a2 T/2 + a3 T^2/3 + a4 T^3/4 + a5 T^4/5 + a6/T
+ *   S/R  = a1 ln T + a2 T + a3 T^2/2 + a4 T^3/3 + a5 T^4/4 + a7
+ * Range selection (reading T3): T <= t_mid -> low set, else high set; no clamping (T4). */
+static const double *nasa_set(const orc_network *net, int i, real_t T) {
+  return (T <= (real_t)net->t_mid[i]) ? net->nasa_lo + 7 * i : net->nasa_hi + 7 * i;
+}
+static real_t nasa_cp(const double *a, real_t T) {
+  return a[0] + a[1] * T + a[2] * T * T + a[3] * T * T * T + a[4] * T * T * T * T;
+}
+static real_t nasa_h(const double *a, real_t T) {
+  return a[0] + a[1] * T / 2 + a[2] * T * T / 3 + a[3] * T * T * T / 4 + a[4] * T * T * T * T / 5 +
+         a[5] / T;
+}
+static real_t nasa_s(const double *a, real_t T) {
+  return a[0] * R_LOG(T) + a[1] * T + a[2] * T * T / 2 + a[3] * T * T * T / 3 +
+         a[4] * T * T * T * T / 4 + a[6];
+}
+static real_t nasa_g(const double *a, real_t T) {
+  return a[0] * (1 - R_LOG(T)) - a[1] * T / 2 - a[2] * T * T / 6 - a[3] * T * T * T / 12 -
+         a[4] * T * T * T * T / 20 + a[5] / T - a[6];
+}
+
+/* Any of cp_R, h_RT, s_R, g_RT may be NULL.  Each is [n_species][ld]. */
+int orc_thermo(const orc_network *net, long ncol, long ld, const double *T, double *cp_R,
+               double *h_RT, double *s_R, double *g_RT) {
+  for (long c = 0; c < ncol; ++c) {
+    real_t Tc = T[c];
+    for (int i = 0; i < net->n_species; ++i) {
+      const double *a = nasa_set(net, i, Tc);
+      if (cp_R) cp_R[(long)i * ld + c] = (double)nasa_cp(a, Tc);
+      if (h_RT) h_RT[(long)i * ld + c] = (double)nasa_h(a, Tc);
+      if (s_R) s_R[(long)i * ld + c] = (double)nasa_s(a, Tc);
+      if (g_RT) g_RT[(long)i * ld + c] = (double)nasa_g(a, Tc);
+    }
+  }
+  return 0;
+}
+
+/* ---------------------------------------------------------------- O2 forward coefficients
+ * PAPER.md:118-122 (Eq. 7): k = alpha T_b^beta exp(-gamma/T_c), T_b = T/300 (Kooij) or T
+ * (modified Arrhenius), T_c = T. */
+static real_t arrhenius(const double *abg, real_t T, real_t t_ref) {
+  return (real_t)abg[0] * R_POW(T / t_ref, (real_t)abg[1]) * R_EXP(-(real_t)abg[2] / T);
+}
+
+/* PAPER.md:148-157 (Eq. 10-12): k0, k_inf as Eq. 7; k = k0[M] / (1 + k0[M]/k_inf).
+ * [M] = P/(k_B T) (north_star).  Troe broadening is not in the paper; reading
+ * F1: log10 F = log10 Fc / (1 + (log10 Pr / N)^2), N = 0.75 - 1.27 log10 Fc, Pr = k0[M]/k_inf;
+ * Fc == 1 is pure Lindemann (Eq. 12). */
+static real_t falloff(const double *inf_abg, const double *low_abg, double fc, real_t T, real_t P,
+                      real_t t_ref) {
+  real_t k0 = arrhenius(low_abg, T, t_ref);
+  real_t kinf = arrhenius(inf_abg, T, t_ref);
+  real_t M = P / (K_BOLTZ * T);
+  real_t Pr = k0 * M / kinf;
+  real_t kL = k0 * M / (1 + Pr);
+  if (fc == 1.0) return kL;
+  real_t lfc = R_LOG10((real_t)fc);
+  real_t N = (real_t)0.75L - (real_t)1.27L * lfc;
+  real_t x = R_LOG10(Pr) / N;
+  real_t F = R_POW((real_t)fc, 1 / (1 + x * x));
+  return kL * F;
+}
+
+/* ---------------------------------------------------------------- O3 reverse coefficients
+ * PAPER.md:225-235 (Eq. 13-15): k_c = k_f / k_r, k_c from the Gibbs energy of reaction
+ * (Tsai et al. 2017 App. E):  K_c = exp(-dG/RT) (P0 / (k_B T))^dnu,
+ *   dG/RT = sum_products G_i/RT - sum_reactants G_i/RT,  dnu = #products - #reactants,
+ * the third body M excluded from both (reading R1).  Photolysis has no reverse (R2). */
+static real_t forward_coeff(const orc_network *net, int r, real_t T, real_t P, const double *J,
+                            int photo_row, long ld, long c) {
+  real_t t_ref = net->t_ref ? (real_t)net->t_ref[r] : (real_t)1;
+  switch (net->type[r]) {
+    case ORC_UNI:
+    case ORC_BI:
+      return arrhenius(net->arrh + 3 * r, T, t_ref);
+    case ORC_FALLOFF:
+      return falloff(net->arrh + 3 * r, net->arrh_low + 3 * r, net->troe_fc[r], T, P, t_ref);
+    default: /* ORC_PHOTO: J supplied by the caller */
+      return (real_t)J[(long)photo_row * ld + c];
+  }
+}
+
+static real_t reverse_coeff(const orc_network *net, int r, real_t kf, real_t T) {
+  if (!net->reversible[r] || net->type[r] == ORC_PHOTO) return 0;
+  real_t dG = 0;
+  int dnu = 0;
+  for (int s = 0; s < 3; ++s) {
+    int i = net->products[3 * r + s];
+    if (i >= 0) {
+      dG += nasa_g(nasa_set(net, i, T), T);
+      ++dnu;
+    }
+  }
+  for (int s = 0; s < 3; ++s) {
+    int i = net->reactants[3 * r + s];
+    if (i >= 0) {
+      dG -= nasa_g(nasa_set(net, i, T), T);
+      --dnu;
+    }
+  }
+  real_t Kc = R_EXP(-dG) * R_POW(P_REF / (K_BOLTZ * T), (real_t)dnu);
+  return kf / Kc;
+}
+
+/* kf, kr: [n_reactions][ld] in USER reaction order.  J: [n_photo][ld]. */
+int orc_rate_coeffs(const orc_network *net, long ncol, long ld, const double *T, const double *P,
+                    const double *J, double *kf, double *kr) {
+  for (long c = 0; c < ncol; ++c) {
+    real_t Tc = T[c], Pc = P[c];
+    int photo_row = 0; /* row p of J is the p-th PHOTO reaction in user order */
+    for (int r = 0; r < net->n_reactions; ++r) {
+      real_t f = forward_coeff(net, r, Tc, Pc, J, photo_row, ld, c);
+      if (net->type[r] == ORC_PHOTO) ++photo_row;
+      real_t b = reverse_coeff(net, r, f, Tc);
+      if (kf) kf[(long)r * ld + c] = (double)f;
+      if (kr) kr[(long)r * ld + c] = (double)b;
+    }
+  }
+  return 0;
+}
+
+/* ---------------------------------------------------------------- O4 rates of progress
+ * q_f = k_f prod_{reactants} n_l, q_r = k_r prod_{products} n_l  (north_star: "k . prod n_reactant";
+ * a repeated index gives n^2, e.g. 2 SO -> SO2 + S). */
+static real_t rate_of(const int *side, real_t k, const double *n, long ld, long c) {
+  real_t q = k;
+  for (int s = 0; s < 3; ++s)
+    if (side[s] >= 0) q *= (real_t)n[(long)side[s] * ld + c];
+  return q;
+}
+
+int orc_rates(const orc_network *net, long ncol, long ld, const double *kf, const double *kr,
+              const double *n, double *qf, double *qr) {
+  for (long c = 0; c < ncol; ++c)
+    for (int r = 0; r < net->n_reactions; ++r) {
+      qf[(long)r * ld + c] = (double)rate_of(net->reactants + 3 * r, kf[(long)r * ld + c], n, ld, c);
+      qr[(long)r * ld + c] = (double)rate_of(net->products + 3 * r, kr[(long)r * ld + c], n, ld, c);
+    }
+  return 0;
+}
+
+/* net stoichiometric coefficient nu_ir = (#i in products) - (#i in reactants) */
+static int nu_of(const orc_network *net, int i, int r) {
+  int v = 0;
+  for (int s = 0; s < 3; ++s) {
+    if (net->products[3 * r + s] == i) ++v;
+    if (net->reactants[3 * r + s] == i) --v;
+  }
+  return v;
+}
+
+/* ---------------------------------------------------------------- O5 production and loss
+ * PAPER.md:53 (Eq. 1): dn_i/dt = P_i - L_i.  dn_i/dt = sum_r nu_ir (q_f,r - q_r,r), summed
+ * in user reaction order, forward term then reverse term.  P_i = sum of the positive terms,
+ * L_i = sum of |negative terms| (a rate, reading S1).  prod, loss may be NULL. */
+/* distinct species of reaction r (both sides), in slot order; returns how many */
+static int distinct_species(const orc_network *net, int r, int *out) {
+  int k = 0;
+  for (int s = 0; s < 6; ++s) {
+    int i = s < 3 ? net->reactants[3 * r + s] : net->products[3 * r + s - 3];
+    if (i < 0) continue;
+    int seen = 0;
+    for (int t = 0; t < k; ++t)
+      if (out[t] == i) seen = 1;
+    if (!seen) out[k++] = i;
+  }
+  return k;
+}
+
+int orc_source(const orc_network *net, long ncol, long ld, const double *kf, const double *kr,
+               const double *n, double *dndt, double *prod, double *loss) {
+  int ns = net->n_species;
+  real_t *sum = (real_t *)malloc(sizeof(real_t) * ns * 3), *sp = sum + ns, *sl = sum + 2 * ns;
+  if (!sum) return -1;
+  for (long c = 0; c < ncol; ++c) {
+    for (int i = 0; i < 3 * ns; ++i) sum[i] = 0;
+    for (int r = 0; r < net->n_reactions; ++r) { /* user reaction order */
+      real_t qf = rate_of(net->reactants + 3 * r, kf[(long)r * ld + c], n, ld, c);
+      real_t qr = rate_of(net->products + 3 * r, kr[(long)r * ld + c], n, ld, c);
+      int sp_r[6], k = distinct_species(net, r, sp_r);
+      for (int t = 0; t < k; ++t) {
+        int i = sp_r[t], nu = nu_of(net, i, r);
+        if (!nu) continue;
+        real_t tf = nu * qf, tr = -nu * qr; /* forward term, then reverse term */
+        sum[i] += tf;
+        sum[i] += tr;
+        if (tf > 0) sp[i] += tf; else sl[i] += -tf;
+        if (tr > 0) sp[i] += tr; else sl[i] += -tr;
+      }
+    }
+    for (int i = 0; i < ns; ++i) {
+      if (dndt) dndt[(long)i * ld + c] = (double)sum[i];
+      if (prod) prod[(long)i * ld + c] = (double)sp[i];
+      if (loss) loss[(long)i * ld + c] = (double)sl[i];
+    }
+  }
+  free(sum);
+  return 0;
+}
+
+/* ---------------------------------------------------------------- O6 Jacobian
+ * d q_f,r / d n_j = k_f,r m_jr n_j^(m_jr - 1) prod_{l != j} n_l^(m_lr), m = multiplicity among the
+ * reactants (never q/n_j: exact at n_j = 0).  k_f, k_r, [M], J do not depend on n (reading J3).
+ * Jac_ij = sum_r nu_ir (d q_f,r/d n_j - d q_r,r/d n_j);
+ * scale_ij = sum_r |nu_ir| (|d q_f,r/d n_j| + |d q_r,r/d n_j|)  (the parity tolerance scale).
+ * dense, scale: [n_species][n_species] row-major for ONE column c. */
+static void add_side_derivatives(const orc_network *net, int r, const int *side, real_t k,
+                                 real_t sign, const double *n, long ld, long c, real_t *dense,
+                                 real_t *scale) {
+  long ns = net->n_species;
+  for (int a = 0; a < 3; ++a) {
+    int j = side[a];
+    if (j < 0) continue;
+    int first = 1, m = 0;
+    for (int b = 0; b < 3; ++b) {
+      if (side[b] == j) {
+        ++m;
+        if (b < a) first = 0;
+      }
+    }
+    if (!first) continue; /* each distinct species j once */
+    real_t d = k * m;     /* k m_j n_j^(m_j-1) prod_{l!=j} n_l^m_l = k m_j prod over all slots but one j-slot */
+    for (int b = 0; b < 3; ++b)
+      if (b != a && side[b] >= 0) d *= (real_t)n[(long)side[b] * ld + c];
+    int sp_r[6], k = distinct_species(net, r, sp_r);
+    for (int t = 0; t < k; ++t) {
+      int i = sp_r[t], nu = nu_of(net, i, r);
+      if (!nu) continue;
+      dense[(long)i * ns + j] += sign * nu * d;
+      scale[(long)i * ns + j] += R_FABS(nu * d);
+    }
+  }
+}
+
+static void jacobian_dense_real(const orc_network *net, long ld, const double *kf, const double *kr,
+                                const double *n, long c, real_t *dense, real_t *scale) {
+  long ns = net->n_species;
+  for (long e = 0; e < ns * ns; ++e) dense[e] = scale[e] = 0;
+  for (int r = 0; r < net->n_reactions; ++r) {
+    add_side_derivatives(net, r, net->reactants + 3 * r, kf[(long)r * ld + c], +1, n, ld, c, dense, scale);
+    add_side_derivatives(net, r, net->products + 3 * r, kr[(long)r * ld + c], -1, n, ld, c, dense, scale);
+  }
+}
+
+int orc_jacobian_dense(const orc_network *net, long ld, const double *kf, const double *kr,
+                       const double *n, long c, double *dense, double *scale) {
+  long ns = net->n_species;
+  real_t *d = (real_t *)malloc(sizeof(real_t) * ns * ns), *s = (real_t *)malloc(sizeof(real_t) * ns * ns);
+  if (!d || !s) return -1;
+  jacobian_dense_real(net, ld, kf, kr, n, c, d, s);
+  for (long e = 0; e < ns * ns; ++e) {
+    dense[e] = (double)d[e];
+    if (scale) scale[e] = (double)s[e];
+  }
+  free(d);
+  free(s);
+  return 0;
+}
+
+/* Pattern values: jac, scale are [nnz][ld].  Returns the number of (entry, column) pairs
+ * OUTSIDE the pattern whose dense value or scale is not exactly 0 (must be 0), or -1. */
+long orc_jacobian(const orc_network *net, long ncol, long ld, const double *kf, const double *kr,
+                  const double *n, const long *row_ptr, const int *col, double *jac, double *scale) {
+  long ns = net->n_species, bad = 0;
+  real_t *d = (real_t *)malloc(sizeof(real_t) * ns * ns), *s = (real_t *)malloc(sizeof(real_t) * ns * ns);
+  unsigned char *in = (unsigned char *)calloc(ns * ns, 1);
+  if (!d || !s || !in) return -1;
+  for (long i = 0; i < ns; ++i)
+    for (long e = row_ptr[i]; e < row_ptr[i + 1]; ++e) in[i * ns + col[e]] = 1;
+  for (long c = 0; c < ncol; ++c) {
+    jacobian_dense_real(net, ld, kf, kr, n, c, d, s);
+    for (long e = 0; e < ns * ns; ++e)
+      if (!in[e] && (d[e] != 0 || s[e] != 0)) ++bad;
+    for (long i = 0; i < ns; ++i)
+      for (long e = row_ptr[i]; e < row_ptr[i + 1]; ++e) {
+        jac[e * ld + c] = (double)d[i * ns + col[e]];
+        if (scale) scale[e * ld + c] = (double)s[i * ns + col[e]];
+      }
+  }
+  free(d);
+  free(s);
+  free(in);
+  return bad;
+}
+
+/* ---------------------------------------------------------------- CSR layouts (readings S2, J1, J2)
+ * Source CSR: row i = species i; entries = all reactions with nu_ir != 0 in ascending user
+ * reaction index; nu in -3..3.  Pass rxn = nu = NULL to get only row_ptr (sizes). */
+long orc_source_csr(const orc_network *net, long *row_ptr, int *rxn, int *nu) {
+  long k = 0;
+  for (int i = 0; i < net->n_species; ++i) {
+    row_ptr[i] = k;
+    for (int r = 0; r < net->n_reactions; ++r) {
+      int v = nu_of(net, i, r);
+      if (!v) continue;
+      if (rxn) rxn[k] = r;
+      if (nu) nu[k] = v;
+      ++k;
+    }
+  }
+  row_ptr[net->n_species] = k;
+  return k;
+}
+
+/* Jacobian pattern: union over reactions of S_r x S_r (S_r = distinct species of reaction r,
+ * both sides) plus the diagonal; rows = species, column indices ascending.  Built from a
+ * dense boolean matrix.  Pass col = NULL to get only row_ptr. */
+long orc_jac_pattern(const orc_network *net, long *row_ptr, int *col) {
+  long ns = net->n_species, k = 0;
+  unsigned char *m = (unsigned char *)calloc(ns * ns, 1);
+  if (!m) return -1;
+  for (long i = 0; i < ns; ++i) m[i * ns + i] = 1;
+  for (int r = 0; r < net->n_reactions; ++r) {
+    int sp[6];
+    for (int s = 0; s < 3; ++s) {
+      sp[s] = net->reactants[3 * r + s];
+      sp[3 + s] = net->products[3 * r + s];
+    }
+    for (int a = 0; a < 6; ++a)
+      for (int b = 0; b < 6; ++b)
+        if (sp[a] >= 0 && sp[b] >= 0) m[(long)sp[a] * ns + sp[b]] = 1;
+  }
+  for (long i = 0; i < ns; ++i) {
+    row_ptr[i] = k;
+    for (long j = 0; j < ns; ++j)
+      if (m[i * ns + j]) {
+        if (col) col[k] = (int)j;
+        ++k;
+      }
+  }
+  row_ptr[ns] = k;
+  free(m);
+  return k;
+}
