@@ -1,0 +1,152 @@
+/* xodiac.h -- C ABI of libxodiac: the batched fp64 chemical source term of the XODIAC 1-D
+ * photochemical kinetics model (arxiv 2512.06729), hand-written CUDA for sm_100a (B200).
+ *
+ * The path (citations are /root/reference/PAPER.md lines):
+ *   a2 NASA-7 thermochemistry  cp/R, H/RT, S/R, G/RT
+ *   a3 forward coefficients    k = alpha T_b^beta exp(-gamma/T)      PAPER.md:116-124 (Eq. 7)
+ *   a4 three-body falloff      Lindemann k0[M]/(1 + k0[M]/k_inf)     PAPER.md:146-159 (Eq. 10-12)
+ *                              x Troe broadening (BASELINE.json north_star; reading F1)
+ *   a5 photolysis              k_f = J (input), dn_A/dt = -k_ph n_A
+ *   a6 reverse coefficients    k_r = k_f / K_c,                      PAPER.md:219-235 (Eq. 13-15)
+ *                              K_c = exp(-dG/RT) (P0/(k_B T))^dnu
+ *   a7 rates of progress       q_f = k_f prod n_reactant, q_r = k_r prod n_product
+ *   a8 production and loss     dn_i/dt = P_i - L_i = sum_r nu_ir (q_f,r - q_r,r)   PAPER.md:53 (Eq. 1)
+ *   a9 Jacobian values         d(dn_i/dt)/dn_j on a fixed CSR pattern (BASELINE.json config 5)
+ *
+ * Conventions
+ *   Units       cgs: T [K], P [dyn cm^-2] (1 bar = 1e6), n [cm^-3], J [s^-1], E/R [K],
+ *               k [s^-1 | cm^3 s^-1 | cm^6 s^-1].  k_B = 1.380649e-16 erg/K, P0 = 1e6 dyn cm^-2.
+ *   Layout      every per-column array is [row][ld], the column index contiguous, ld >= ncol the
+ *               row pitch in elements.  A column is one (atmosphere, layer) pair.
+ *   Order       kf, kr rows are the USER's reaction order.  Row p of J is the p-th XOD_PHOTO
+ *               reaction in user order.  The type-sorted order is internal (xod_network_perm).
+ *   Memory      xod_network_desc pointers are HOST memory, copied by create.  Every pointer of a
+ *               compute call is DEVICE memory owned by the caller, except in the *_host call.
+ *   Streams     `stream` is a cudaStream_t passed as void* (NULL = default stream).  Compute
+ *               calls only enqueue work and never synchronise; the *_host call synchronises.
+ *   Errors      argument problems return synchronously with nothing enqueued; xod_last_error()
+ *               (thread-local) says what was wrong.  IEEE overflow/underflow in results (k_r
+ *               beyond the double range, reading R5) is not an error.
+ *   Threads     a network is immutable after create; concurrent calls on different streams are
+ *               legal if each has its own workspace.
+ *   No CPU fallback exists: without a CUDA device every compute call returns XOD_ERR_CUDA.
+ */
+#ifndef XODIAC_H
+#define XODIAC_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct xod_network xod_network; /* opaque; owns its device tables */
+
+typedef enum {
+  XOD_OK = 0,
+  XOD_ERR_INVALID_ARG = 1, /* NULL pointer, bad size, index out of range, bad type, Fc not in (0,1] ... */
+  XOD_ERR_UNBALANCED = 2,  /* a reaction does not conserve an element (names the reaction) */
+  XOD_ERR_ALLOC = 3,
+  XOD_ERR_CUDA = 4,        /* no device, or a launch / copy failed */
+  XOD_ERR_WORKSPACE = 5    /* workspace NULL or smaller than xod_*_workspace_bytes */
+} xod_status;
+
+/* Reaction categories of PAPER.md:105; also the internal sort key (north_star: "sorts reactions by
+ * type (unimolecular, bimolecular, three-body falloff, photolysis)").  XOD_UNI / XOD_BI are thermal
+ * non-falloff reactions with one / two-or-three listed reactants. */
+enum { XOD_UNI = 0, XOD_BI = 1, XOD_FALLOFF = 2, XOD_PHOTO = 3 };
+
+enum { XOD_FLAG_SKIP_BALANCE_CHECK = 1u };
+
+typedef struct {
+  int32_t n_species, n_elements, n_reactions;
+  const int32_t *composition; /* [n_species][n_elements] atoms per element; may be negative (charge
+                                 carried as an extra "element", cf. C -> C+ + e-) */
+  const double *nasa_lo;      /* [n_species][7] a1..a7, low-temperature range */
+  const double *nasa_hi;      /* [n_species][7] a1..a7, high-temperature range */
+  const double *t_mid;        /* [n_species]; T <= t_mid uses nasa_lo, else nasa_hi */
+  const int32_t *type;        /* [n_reactions] XOD_* */
+  const int32_t *reactants;   /* [n_reactions][3], -1 padded; a stoichiometric 2 is the index repeated */
+  const int32_t *products;    /* [n_reactions][3], -1 padded; the third body M is never listed */
+  const uint8_t *reversible;  /* [n_reactions]; must be 0 for XOD_PHOTO */
+  const double *arrh;         /* [n_reactions][3] alpha, beta, gamma (Eq. 7); k_inf for XOD_FALLOFF
+                                 (Eq. 11); ignored for XOD_PHOTO */
+  const double *arrh_low;     /* [n_reactions][3] alpha0, beta0, gamma0 (Eq. 10); XOD_FALLOFF only */
+  const double *troe_fc;      /* [n_reactions] Fc in (0,1]; 1 = pure Lindemann (Eq. 12); XOD_FALLOFF only */
+  const double *t_ref;        /* [n_reactions] 1 = modified Arrhenius, 300 = Kooij (Eq. 7); NULL = all 1 */
+  uint32_t flags;             /* XOD_FLAG_* */
+} xod_network_desc;
+
+/* a0: validate, sort by type, build the SoA parameter tables, the source CSR and the Jacobian CSR
+ * with its term lists, and upload them to `cuda_device`.  With cuda_device < 0 only the host side
+ * is built (introspection works, compute calls fail with XOD_ERR_CUDA). */
+xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod_network **out);
+void xod_network_destroy(xod_network *net);
+const char *xod_last_error(void);
+
+/* ---- introspection: host outputs, caller-allocated; any output pointer may be NULL */
+xod_status xod_network_sizes(const xod_network *net, int32_t *n_species, int32_t *n_reactions,
+                             int32_t *n_photo, int64_t *nnz_source, int64_t *nnz_jac,
+                             int64_t *n_jac_terms);
+/* packed (type-sorted, stable) position -> user reaction index, [n_reactions] */
+xod_status xod_network_perm(const xod_network *net, int32_t *packed_to_user);
+/* row p of J -> user reaction index, [n_photo] */
+xod_status xod_network_photo_index(const xod_network *net, int32_t *user_rxn_of_photo_row);
+/* source CSR (reading S2): row i = species i; entries = reactions with nu_ir != 0 in
+ * ascending USER reaction index; row_ptr [n_species+1], rxn and nu [nnz_source] */
+xod_status xod_network_source_csr(const xod_network *net, int64_t *row_ptr, int32_t *rxn, int32_t *nu);
+/* Jacobian pattern (readings J1, J2): union over reactions of (distinct species)^2 plus the
+ * diagonal; rows = species, ascending column indices; row_ptr [n_species+1], col [nnz_jac] */
+xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int32_t *col);
+
+/* ---- tuning knobs (optional; defaults are chosen for B200) */
+enum { XOD_TUNE_CHUNK_COLS = 0 /* columns per pipeline chunk of the fused source call */ };
+xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
+
+/* ---- a2: NASA-7 thermochemistry.  T [ld]; each output [n_species][ld], any may be NULL. */
+xod_status xod_thermo(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                      double *cp_R, double *h_RT, double *s_R, double *g_RT, void *stream);
+
+/* ---- a1, a3-a6: forward and reverse rate coefficients.  T, P [ld]; J [n_photo][ld] (may be NULL
+ * if n_photo == 0); kf, kr [n_reactions][ld] in user order, either may be NULL.  kr rows of
+ * irreversible and photolysis reactions are 0. */
+size_t xod_rate_coeffs_workspace_bytes(const xod_network *net, int64_t ncol);
+xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                           const double *P, const double *J, double *kf, double *kr,
+                           void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- a7-a8: dn/dt from stored coefficients.  n [n_species][ld]; dndt [n_species][ld];
+ * prod, loss optional (both or neither): P_i = sum of positive terms, L_i = sum of |negative
+ * terms|, dn/dt = P - L. */
+size_t xod_source_workspace_bytes(const xod_network *net, int64_t ncol);
+xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
+                      const double *kr, const double *n, double *dndt, double *prod, double *loss,
+                      void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- a1-a8 fused: (T, P, J, n) -> dn/dt without k_f, k_r ever reaching HBM (the headline path). */
+size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol);
+xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                            const double *P, const double *J, const double *n, double *dndt,
+                            double *prod, double *loss, void *workspace, size_t workspace_bytes,
+                            void *stream);
+
+/* ---- a9: Jacobian values jac[e][col], e over the pattern of xod_network_jac_pattern. */
+xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
+                        const double *kr, const double *n, double *jac, void *stream);
+
+/* ---- end-to-end convenience: the fused call on HOST buffers (pinned or pageable).  Copies
+ * T, P, J, n to the device, runs xod_source_fused, copies dndt back and synchronises.  Device
+ * staging buffers are owned by the network and grown on demand (not thread-safe on one network). */
+xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                                 const double *P, const double *J, const double *n, double *dndt);
+
+/* ---- measurement helper: sustained DFMA issue rate of the device (dependent-chain-free FMA
+ * loop on every SM), used as the FP64 roofline denominator.  Returns fused multiply-adds per
+ * second (flops = 2x) measured over `iters` launches with CUDA events; synchronises. */
+xod_status xod_probe_fp64_peak(int cuda_device, int32_t iters, double *dfma_per_second);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* XODIAC_H */

@@ -1,0 +1,205 @@
+"""Thin ctypes binding of libxodiac.so: the same names as include/xodiac.h, argument marshalling
+only.  Device buffers are torch tensors (fp64, CUDA); every step of the path runs in the CUDA
+kernels of the library.  There is no CPU fallback: a missing library raises at first use."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libxodiac.so")
+_lib = None
+
+XOD_OK = 0
+XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
+XOD_FLAG_SKIP_BALANCE_CHECK = 1
+XOD_TUNE_CHUNK_COLS = 0
+STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
+                4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
+
+EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_network_sizes",
+           "xod_network_perm", "xod_network_photo_index", "xod_network_source_csr",
+           "xod_network_jac_pattern", "xod_network_tune", "xod_thermo",
+           "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
+           "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
+           "xod_source_fused_host", "xod_probe_fp64_peak"]
+
+
+class XodError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, status), message))
+        self.status = status
+
+
+class _Desc(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("n_elements", C.c_int32), ("n_reactions", C.c_int32),
+                ("composition", C.c_void_p), ("nasa_lo", C.c_void_p), ("nasa_hi", C.c_void_p),
+                ("t_mid", C.c_void_p), ("type", C.c_void_p), ("reactants", C.c_void_p),
+                ("products", C.c_void_p), ("reversible", C.c_void_p), ("arrh", C.c_void_p),
+                ("arrh_low", C.c_void_p), ("troe_fc", C.c_void_p), ("t_ref", C.c_void_p),
+                ("flags", C.c_uint32)]
+
+
+def lib():
+    """Load libxodiac.so (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError("libxodiac.so is missing: run `python -m paper_2512_06729_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        L.xod_last_error.restype = C.c_char_p
+        for name in ("xod_rate_coeffs_workspace_bytes", "xod_source_workspace_bytes",
+                     "xod_source_fused_workspace_bytes"):
+            getattr(L, name).restype = C.c_size_t
+            getattr(L, name).argtypes = [C.c_void_p, C.c_int64]
+        L.xod_network_destroy.restype = None
+        L.xod_network_destroy.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _check(st):
+    if st != XOD_OK:
+        raise XodError(st, lib().xod_last_error().decode())
+
+
+def _np(a, dtype):
+    return None if a is None else np.ascontiguousarray(a, dtype=dtype)
+
+
+def _hp(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def _dp(t):
+    """Device pointer of a torch tensor (fp64, CUDA, contiguous rows) or None."""
+    if t is None:
+        return None
+    assert t.is_cuda and t.dtype.is_floating_point and t.element_size() == 8 and t.is_contiguous()
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+class Network:
+    """xod_network handle.  `net` is any object with the attributes of synth.Network."""
+
+    def __init__(self, net, device=0, flags=0):
+        L = lib()
+        keep = dict(
+            composition=_np(net.composition, np.int32), nasa_lo=_np(net.nasa_lo, np.float64),
+            nasa_hi=_np(net.nasa_hi, np.float64), t_mid=_np(net.t_mid, np.float64),
+            type=_np(net.type, np.int32), reactants=_np(net.reactants, np.int32),
+            products=_np(net.products, np.int32), reversible=_np(net.reversible, np.uint8),
+            arrh=_np(net.arrh, np.float64), arrh_low=_np(getattr(net, "arrh_low", None), np.float64),
+            troe_fc=_np(getattr(net, "troe_fc", None), np.float64),
+            t_ref=_np(getattr(net, "t_ref", None), np.float64))
+        ns, ne = keep["composition"].shape
+        d = _Desc(ns, ne, keep["type"].shape[0], *[_hp(keep[k]) for k in (
+            "composition", "nasa_lo", "nasa_hi", "t_mid", "type", "reactants", "products", "reversible",
+            "arrh", "arrh_low", "troe_fc", "t_ref")], flags)
+        h = C.c_void_p()
+        _check(L.xod_network_create(C.byref(d), C.c_int(device), C.byref(h)))
+        self._h = h
+        self.device = device
+        v = [C.c_int32(), C.c_int32(), C.c_int32(), C.c_int64(), C.c_int64(), C.c_int64()]
+        _check(L.xod_network_sizes(h, *[C.byref(x) for x in v]))
+        (self.n_species, self.n_reactions, self.n_photo, self.nnz_source, self.nnz_jac,
+         self.n_jac_terms) = [x.value for x in v]
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().xod_network_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- introspection
+    def perm(self):
+        out = np.zeros(self.n_reactions, dtype=np.int32)
+        _check(lib().xod_network_perm(self._h, _hp(out)))
+        return out
+
+    def photo_index(self):
+        out = np.zeros(self.n_photo, dtype=np.int32)
+        _check(lib().xod_network_photo_index(self._h, _hp(out)))
+        return out
+
+    def source_csr(self):
+        rp = np.zeros(self.n_species + 1, dtype=np.int64)
+        rxn, nu = np.zeros(self.nnz_source, dtype=np.int32), np.zeros(self.nnz_source, dtype=np.int32)
+        _check(lib().xod_network_source_csr(self._h, _hp(rp), _hp(rxn), _hp(nu)))
+        return rp, rxn, nu
+
+    def jac_pattern(self):
+        rp = np.zeros(self.n_species + 1, dtype=np.int64)
+        col = np.zeros(self.nnz_jac, dtype=np.int32)
+        _check(lib().xod_network_jac_pattern(self._h, _hp(rp), _hp(col)))
+        return rp, col
+
+    def tune(self, knob, value):
+        _check(lib().xod_network_tune(self._h, C.c_int32(knob), C.c_int64(value)))
+
+    # ---- workspace sizes
+    def rate_coeffs_workspace_bytes(self, ncol):
+        return lib().xod_rate_coeffs_workspace_bytes(self._h, ncol)
+
+    def source_workspace_bytes(self, ncol):
+        return lib().xod_source_workspace_bytes(self._h, ncol)
+
+    def source_fused_workspace_bytes(self, ncol):
+        return lib().xod_source_fused_workspace_bytes(self._h, ncol)
+
+    # ---- compute calls (device tensors)
+    def thermo(self, ncol, ld, T, cp_R=None, h_RT=None, s_R=None, g_RT=None, stream=None):
+        _check(lib().xod_thermo(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(T), _dp(cp_R), _dp(h_RT),
+                                _dp(s_R), _dp(g_RT), _stream(stream)))
+
+    def rate_coeffs(self, ncol, ld, T, P, J, kf, kr, workspace, stream=None):
+        _check(lib().xod_rate_coeffs(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(T), _dp(P), _dp(J),
+                                     _dp(kf), _dp(kr), _dp(workspace),
+                                     C.c_size_t(0 if workspace is None else workspace.numel() * 8),
+                                     _stream(stream)))
+
+    def source(self, ncol, ld, kf, kr, n, dndt, prod=None, loss=None, workspace=None, stream=None):
+        _check(lib().xod_source(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(kf), _dp(kr), _dp(n),
+                                _dp(dndt), _dp(prod), _dp(loss), _dp(workspace),
+                                C.c_size_t(0 if workspace is None else workspace.numel() * 8),
+                                _stream(stream)))
+
+    def source_fused(self, ncol, ld, T, P, J, n, dndt, prod=None, loss=None, workspace=None, stream=None):
+        _check(lib().xod_source_fused(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(T), _dp(P), _dp(J),
+                                      _dp(n), _dp(dndt), _dp(prod), _dp(loss), _dp(workspace),
+                                      C.c_size_t(0 if workspace is None else workspace.numel() * 8),
+                                      _stream(stream)))
+
+    def jacobian(self, ncol, ld, kf, kr, n, jac, stream=None):
+        _check(lib().xod_jacobian(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(kf), _dp(kr), _dp(n),
+                                  _dp(jac), _stream(stream)))
+
+    # ---- end to end on HOST buffers (numpy arrays or pinned torch CPU tensors)
+    def source_fused_host(self, ncol, ld, T, P, J, n, dndt):
+        def hp(a):
+            if a is None:
+                return None
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float64 and a.flags.c_contiguous
+                return C.c_void_p(a.ctypes.data)
+            assert (not a.is_cuda) and a.element_size() == 8 and a.is_contiguous()
+            return C.c_void_p(a.data_ptr())
+        _check(lib().xod_source_fused_host(self._h, C.c_int64(ncol), C.c_int64(ld), hp(T), hp(P), hp(J),
+                                           hp(n), hp(dndt)))
+
+
+def probe_fp64_peak(device=0, iters=20):
+    out = C.c_double()
+    _check(lib().xod_probe_fp64_peak(C.c_int(device), C.c_int32(iters), C.byref(out)))
+    return out.value

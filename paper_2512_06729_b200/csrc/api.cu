@@ -1,0 +1,454 @@
+// api.cu -- the C ABI of include/xodiac.h: argument checks, workspace carving, kernel launches
+// on the caller's stream.  No host synchronisation in any compute call except *_host.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "kernels.cuh"
+
+using namespace xod;
+
+namespace {
+
+thread_local std::string g_err;
+
+xod_status fail(xod_status s, const std::string &m) {
+  g_err = m;
+  return s;
+}
+xod_status cuda_fail(cudaError_t e, const char *where) {
+  g_err = std::string(where) + ": " + cudaGetErrorString(e);
+  return XOD_ERR_CUDA;
+}
+#define XOD_CUDA(call)                                       \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call);      \
+  } while (0)
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+template <class T>
+xod_status upload(xod_network *net, const std::vector<T> &v, const T **dst) {
+  void *p = nullptr;
+  size_t bytes = std::max<size_t>(v.size() * sizeof(T), 16);
+  XOD_CUDA(cudaMalloc(&p, bytes));
+  net->dev_allocs.push_back(p);
+  if (!v.empty()) XOD_CUDA(cudaMemcpy(p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+  *dst = static_cast<const T *>(p);
+  return XOD_OK;
+}
+
+const double kLog2Kb = (double)std::log2(1.380649e-16L);
+
+constexpr int64_t kDefaultChunk = 1024;  // columns per pipeline chunk: q chunk = nr*1024*8 B stays in L2
+
+int64_t chunk_cols(const xod_network *net, int64_t ncol) {
+  int64_t c = net->chunk_cols > 0 ? net->chunk_cols : kDefaultChunk;
+  c = round_up(c, 32);
+  return std::min<int64_t>(c, round_up(std::max<int64_t>(ncol, 1), 32));
+}
+
+// carve the workspace: [l2T | invT | lM | u (ns rows) | q (nr rows) | qr (nr rows, optional)]
+size_t scratch_bytes(const xod_network *net, int64_t ldw, bool need_u, bool need_q, bool pl) {
+  size_t rows = 0;
+  if (need_u) rows += 3 + (size_t)net->h.ns;
+  if (need_q) rows += (size_t)net->h.nr * (pl ? 2 : 1);
+  return rows * (size_t)ldw * sizeof(double) + 256;
+}
+ChunkScratch carve(const xod_network *net, void *ws, int64_t ldw, bool need_u, bool need_q, bool pl) {
+  ChunkScratch s{};
+  uintptr_t a = (reinterpret_cast<uintptr_t>(ws) + 255) & ~uintptr_t(255);
+  double *p = reinterpret_cast<double *>(a);
+  s.ldw = ldw;
+  if (need_u) {
+    s.l2T = p, p += ldw;
+    s.invT = p, p += ldw;
+    s.lM = p, p += ldw;
+    s.u = p, p += (size_t)net->h.ns * ldw;
+  }
+  if (need_q) {
+    s.q = p, p += (size_t)net->h.nr * ldw;
+    if (pl) s.qr = p;
+  }
+  return s;
+}
+
+xod_status check_common(const xod_network *net, int64_t ncol, int64_t ld) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  if (ncol < 0) return fail(XOD_ERR_INVALID_ARG, "ncol < 0");
+  if (ld < ncol) return fail(XOD_ERR_INVALID_ARG, "ld < ncol");
+  if (net->device < 0) return fail(XOD_ERR_CUDA, "network was created without a CUDA device");
+  int cur = -1;
+  XOD_CUDA(cudaGetDevice(&cur));
+  if (cur != net->device) XOD_CUDA(cudaSetDevice(net->device));
+  return XOD_OK;
+}
+
+// reactions per warp task: aim at ~2 resident waves of warps over the whole chip
+int pick_rw(int nr, int64_t ncg) {
+  const int64_t target = 148LL * 32 * 2;
+  int64_t rw = ((int64_t)nr * ncg + target - 1) / target;
+  return (int)std::min<int64_t>(std::max<int64_t>(rw, 8), 128);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *xod_last_error(void) { return g_err.c_str(); }
+
+xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod_network **out) {
+  if (!out) return fail(XOD_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  xod_network *net = new (std::nothrow) xod_network;
+  if (!net) return fail(XOD_ERR_ALLOC, "out of host memory");
+  std::string err;
+  xod_status st;
+  try {
+    st = pack_network(desc, net->h, err);
+  } catch (const std::bad_alloc &) {
+    delete net;
+    return fail(XOD_ERR_ALLOC, "out of host memory while packing");
+  }
+  if (st != XOD_OK) {
+    delete net;
+    return fail(st, err);
+  }
+  net->device = cuda_device;
+  if (cuda_device >= 0) {
+    int prev = -1;
+    cudaError_t e = cudaGetDevice(&prev);
+    if (e == cudaSuccess) e = cudaSetDevice(cuda_device);
+    if (e != cudaSuccess) {
+      delete net;
+      return cuda_fail(e, "cudaSetDevice");
+    }
+    HostTables &h = net->h;
+    DevTables &d = net->d;
+    d.ns = h.ns, d.nr = h.nr, d.n_photo = h.n_photo;
+    d.uni_begin = h.uni_begin, d.bi_begin = h.bi_begin, d.fo_begin = h.fo_begin, d.ph_begin = h.ph_begin;
+    d.n_src_tasks = (int32_t)(h.src_seg.size() / kSrcWarpsPerCta);
+    d.nnz_jac = (int64_t)h.jac_col.size();
+    st = XOD_OK;
+#define UP(vec, field) if (st == XOD_OK) st = upload(net, h.vec, &d.field)
+    UP(c0, c0); UP(c1, c1); UP(c2, c2);
+    UP(l0, l0); UP(l1, l1); UP(l2, l2); UP(fcl, fcl); UP(cN, cN);
+    UP(sp, sp); UP(flags, flags); UP(packed_to_user, user); UP(photo_row, photo_row);
+    UP(nasa, nasa); UP(nasa_l2, nasa_l2); UP(tmid, tmid);
+    UP(src_rxn_packed, src_rxn); UP(src_nu_f, src_nu); UP(src_seg, src_seg);
+    UP(jac_term_ptr, jac_term_ptr); UP(jac_terms, jac_terms);
+#undef UP
+    if (prev >= 0 && prev != cuda_device) cudaSetDevice(prev);
+    if (st != XOD_OK) {
+      std::string keep = g_err;
+      xod_network_destroy(net);
+      g_err = keep;
+      return st;
+    }
+  }
+  *out = net;
+  return XOD_OK;
+}
+
+void xod_network_destroy(xod_network *net) {
+  if (!net) return;
+  for (void *p : net->dev_allocs) cudaFree(p);
+  if (net->stage) cudaFree(net->stage);
+  delete net;
+}
+
+xod_status xod_network_sizes(const xod_network *net, int32_t *n_species, int32_t *n_reactions,
+                             int32_t *n_photo, int64_t *nnz_source, int64_t *nnz_jac,
+                             int64_t *n_jac_terms) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  if (n_species) *n_species = net->h.ns;
+  if (n_reactions) *n_reactions = net->h.nr;
+  if (n_photo) *n_photo = net->h.n_photo;
+  if (nnz_source) *nnz_source = (int64_t)net->h.src_rxn_user.size();
+  if (nnz_jac) *nnz_jac = (int64_t)net->h.jac_col.size();
+  if (n_jac_terms) *n_jac_terms = (int64_t)net->h.jac_terms.size();
+  return XOD_OK;
+}
+
+xod_status xod_network_perm(const xod_network *net, int32_t *packed_to_user) {
+  if (!net || !packed_to_user) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
+  std::memcpy(packed_to_user, net->h.packed_to_user.data(), net->h.packed_to_user.size() * sizeof(int32_t));
+  return XOD_OK;
+}
+
+xod_status xod_network_photo_index(const xod_network *net, int32_t *user_rxn_of_photo_row) {
+  if (!net || !user_rxn_of_photo_row) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
+  std::memcpy(user_rxn_of_photo_row, net->h.photo_user.data(), net->h.photo_user.size() * sizeof(int32_t));
+  return XOD_OK;
+}
+
+xod_status xod_network_source_csr(const xod_network *net, int64_t *row_ptr, int32_t *rxn, int32_t *nu) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  const HostTables &h = net->h;
+  if (row_ptr) std::memcpy(row_ptr, h.src_ptr.data(), h.src_ptr.size() * sizeof(int64_t));
+  if (rxn) std::memcpy(rxn, h.src_rxn_user.data(), h.src_rxn_user.size() * sizeof(int32_t));
+  if (nu) std::memcpy(nu, h.src_nu.data(), h.src_nu.size() * sizeof(int32_t));
+  return XOD_OK;
+}
+
+xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int32_t *col) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  const HostTables &h = net->h;
+  if (row_ptr) std::memcpy(row_ptr, h.jac_ptr.data(), h.jac_ptr.size() * sizeof(int64_t));
+  if (col) std::memcpy(col, h.jac_col.data(), h.jac_col.size() * sizeof(int32_t));
+  return XOD_OK;
+}
+
+xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  if (knob == XOD_TUNE_CHUNK_COLS) {
+    if (value < 0) return fail(XOD_ERR_INVALID_ARG, "chunk columns must be >= 0");
+    net->chunk_cols = value;
+    return XOD_OK;
+  }
+  return fail(XOD_ERR_INVALID_ARG, "unknown tuning knob");
+}
+
+// ---------------------------------------------------------------------------- compute calls
+
+xod_status xod_thermo(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                      double *cp_R, double *h_RT, double *s_R, double *g_RT, void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0) return XOD_OK;
+  if (!T) return fail(XOD_ERR_INVALID_ARG, "T is NULL");
+  if (!cp_R && !h_RT && !s_R && !g_RT) return XOD_OK;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int64_t gx = (ncol + 127) / 128;
+  // enough CTAs to fill the chip even for one atmosphere: split the species over blockIdx.y
+  int spb = net->h.ns;
+  while (spb > 4 && gx * ((net->h.ns + spb - 1) / spb) < 148 * 8) spb = (spb + 1) / 2;
+  dim3 grid((unsigned)gx, (unsigned)((net->h.ns + spb - 1) / spb));
+  k_thermo<<<grid, 128, 0, s>>>(net->d, ncol, ld, T, cp_R, h_RT, s_R, g_RT, spb);
+  XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+size_t xod_rate_coeffs_workspace_bytes(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0) return 0;
+  return scratch_bytes(net, chunk_cols(net, ncol), true, false, false);
+}
+
+}  // extern "C"
+
+namespace {
+
+xod_status launch_prologue(const xod_network *net, int64_t ncol, int64_t col0, int64_t ncg,
+                           const double *T, const double *P, const ChunkScratch &w, cudaStream_t s) {
+  int split = 1;
+  while (split < 64 && ncg * split < 148 * 2 && split * 8 < net->h.ns) split *= 2;
+  dim3 grid((unsigned)ncg, (unsigned)split);
+  k_prologue<<<grid, 256, 0, s>>>(net->d, ncol, col0, T, P, w, kLog2Kb);
+  XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+template <int MODE>
+xod_status launch_rates(const xod_network *net, int64_t ncol, int64_t col0, int64_t ld, int64_t ncg,
+                        const ChunkScratch &w, const double *J, const double *n, double *kf, double *kr,
+                        cudaStream_t s) {
+  const int rw = pick_rw(net->h.nr, ncg);
+  const int64_t nslices = (net->h.nr + rw - 1) / rw;
+  const int64_t ntasks = nslices * ncg;
+  const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, 148LL * 16);
+  k_rates<MODE><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, J, n, kf, kr, rw, (int)ncg, ntasks);
+  XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+template <bool PL>
+xod_status launch_source(const xod_network *net, int64_t ncol, int64_t col0, int64_t ld, int64_t ncg,
+                         const ChunkScratch &w, double *dndt, double *prod, double *loss, cudaStream_t s) {
+  dim3 grid((unsigned)net->d.n_src_tasks, (unsigned)ncg);
+  k_source<PL><<<grid, 256, 0, s>>>(net->d, ncol, col0, ld, w, dndt, prod, loss);
+  XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                           const double *P, const double *J, double *kf, double *kr,
+                           void *workspace, size_t workspace_bytes, void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0 || net->h.nr == 0) return XOD_OK;
+  if (!T || !P) return fail(XOD_ERR_INVALID_ARG, "T or P is NULL");
+  if (net->h.n_photo > 0 && !J) return fail(XOD_ERR_INVALID_ARG, "J is NULL but the network has photolysis reactions");
+  if (!kf && !kr) return XOD_OK;
+  if (!workspace || workspace_bytes < xod_rate_coeffs_workspace_bytes(net, ncol))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_rate_coeffs_workspace_bytes");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int64_t ldw = chunk_cols(net, ncol);
+  ChunkScratch w = carve(net, workspace, ldw, true, false, false);
+  for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {
+    const int64_t nc = std::min(ldw, ncol - col0), ncg = (nc + 31) / 32;
+    if ((st = launch_prologue(net, ncol, col0, ncg, T, P, w, s)) != XOD_OK) return st;
+    if ((st = launch_rates<MODE_K>(net, ncol, col0, ld, ncg, w, J, nullptr, kf, kr, s)) != XOD_OK) return st;
+  }
+  return XOD_OK;
+}
+
+size_t xod_source_workspace_bytes(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0) return 0;
+  return scratch_bytes(net, chunk_cols(net, ncol), false, true, true);
+}
+
+xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
+                      const double *kr, const double *n, double *dndt, double *prod, double *loss,
+                      void *workspace, size_t workspace_bytes, void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0) return XOD_OK;
+  if (!n || !dndt) return fail(XOD_ERR_INVALID_ARG, "n or dndt is NULL");
+  if (net->h.nr > 0 && (!kf || !kr)) return fail(XOD_ERR_INVALID_ARG, "kf or kr is NULL");
+  if ((prod == nullptr) != (loss == nullptr)) return fail(XOD_ERR_INVALID_ARG, "prod and loss must be given together");
+  if (!workspace || workspace_bytes < xod_source_workspace_bytes(net, ncol))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_workspace_bytes");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const bool pl = prod != nullptr;
+  const int64_t ldw = chunk_cols(net, ncol);
+  ChunkScratch w = carve(net, workspace, ldw, false, true, pl);
+  for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {
+    const int64_t nc = std::min(ldw, ncol - col0), ncg = (nc + 31) / 32;
+    if (net->h.nr > 0) {
+      const int rw = pick_rw(net->h.nr, ncg);
+      const int64_t ntasks = (int64_t)((net->h.nr + rw - 1) / rw) * ncg;
+      const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, 148LL * 16);
+      if (pl)
+        k_rates_from_k<MODE_QSEP><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, kf, kr, n, rw, (int)ncg, ntasks);
+      else
+        k_rates_from_k<MODE_QNET><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, kf, kr, n, rw, (int)ncg, ntasks);
+      XOD_CUDA(cudaGetLastError());
+    }
+    st = pl ? launch_source<true>(net, ncol, col0, ld, ncg, w, dndt, prod, loss, s)
+            : launch_source<false>(net, ncol, col0, ld, ncg, w, dndt, prod, loss, s);
+    if (st != XOD_OK) return st;
+  }
+  return XOD_OK;
+}
+
+size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0) return 0;
+  return scratch_bytes(net, chunk_cols(net, ncol), true, true, true);
+}
+
+xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                            const double *P, const double *J, const double *n, double *dndt,
+                            double *prod, double *loss, void *workspace, size_t workspace_bytes,
+                            void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0) return XOD_OK;
+  if (!T || !P || !n || !dndt) return fail(XOD_ERR_INVALID_ARG, "T, P, n or dndt is NULL");
+  if (net->h.n_photo > 0 && !J) return fail(XOD_ERR_INVALID_ARG, "J is NULL but the network has photolysis reactions");
+  if ((prod == nullptr) != (loss == nullptr)) return fail(XOD_ERR_INVALID_ARG, "prod and loss must be given together");
+  if (!workspace || workspace_bytes < xod_source_fused_workspace_bytes(net, ncol))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_fused_workspace_bytes");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const bool pl = prod != nullptr;
+  const int64_t ldw = chunk_cols(net, ncol);
+  ChunkScratch w = carve(net, workspace, ldw, true, true, pl);
+  for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {
+    const int64_t nc = std::min(ldw, ncol - col0), ncg = (nc + 31) / 32;
+    if (net->h.nr > 0) {
+      if ((st = launch_prologue(net, ncol, col0, ncg, T, P, w, s)) != XOD_OK) return st;
+      st = pl ? launch_rates<MODE_QSEP>(net, ncol, col0, ld, ncg, w, J, n, nullptr, nullptr, s)
+              : launch_rates<MODE_QNET>(net, ncol, col0, ld, ncg, w, J, n, nullptr, nullptr, s);
+      if (st != XOD_OK) return st;
+    }
+    st = pl ? launch_source<true>(net, ncol, col0, ld, ncg, w, dndt, prod, loss, s)
+            : launch_source<false>(net, ncol, col0, ld, ncg, w, dndt, prod, loss, s);
+    if (st != XOD_OK) return st;
+  }
+  return XOD_OK;
+}
+
+xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
+                        const double *kr, const double *n, double *jac, void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0) return XOD_OK;
+  if (!n || !jac) return fail(XOD_ERR_INVALID_ARG, "n or jac is NULL");
+  if (net->h.nr > 0 && (!kf || !kr)) return fail(XOD_ERR_INVALID_ARG, "kf or kr is NULL");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int64_t ncg = (ncol + 31) / 32;
+  if (ncg > 65535) return fail(XOD_ERR_INVALID_ARG, "ncol too large for one xod_jacobian call (max 2097120)");
+  const int64_t want = (net->d.nnz_jac + 7) / 8;
+  const int64_t gx = std::max<int64_t>(1, std::min<int64_t>(want, std::max<int64_t>(1, 148LL * 64 / ncg)));
+  dim3 grid((unsigned)gx, (unsigned)ncg);
+  k_jacobian<<<grid, 256, 0, s>>>(net->d, ncol, ld, kf, kr, n, jac);
+  XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, const double *T,
+                                 const double *P, const double *J, const double *n, double *dndt) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0) return XOD_OK;
+  if (!T || !P || !n || !dndt) return fail(XOD_ERR_INVALID_ARG, "T, P, n or dndt is NULL");
+  if (net->h.n_photo > 0 && !J) return fail(XOD_ERR_INVALID_ARG, "J is NULL but the network has photolysis reactions");
+  const size_t ns = net->h.ns, nph = net->h.n_photo, pitch = (size_t)ld * sizeof(double);
+  const size_t ws = xod_source_fused_workspace_bytes(net, ncol);
+  // staging layout: T | P | J | n | dndt | workspace
+  const size_t rows = 2 + nph + 2 * ns;
+  const size_t need = rows * pitch + ws + 512;
+  if (net->stage_bytes < need) {
+    if (net->stage) cudaFree(net->stage);
+    net->stage = nullptr, net->stage_bytes = 0;
+    XOD_CUDA(cudaMalloc(&net->stage, need));
+    net->stage_bytes = need;
+  }
+  double *dT = static_cast<double *>(net->stage), *dP = dT + ld, *dJ = dP + ld, *dn = dJ + nph * ld,
+         *dd = dn + ns * ld;
+  void *dws = dd + ns * ld;
+  cudaStream_t s = nullptr;
+  XOD_CUDA(cudaMemcpyAsync(dT, T, pitch, cudaMemcpyHostToDevice, s));
+  XOD_CUDA(cudaMemcpyAsync(dP, P, pitch, cudaMemcpyHostToDevice, s));
+  if (nph) XOD_CUDA(cudaMemcpyAsync(dJ, J, nph * pitch, cudaMemcpyHostToDevice, s));
+  XOD_CUDA(cudaMemcpyAsync(dn, n, ns * pitch, cudaMemcpyHostToDevice, s));
+  st = xod_source_fused(net, ncol, ld, dT, dP, dJ, dn, dd, nullptr, nullptr, dws, ws + 256, s);
+  if (st != XOD_OK) return st;
+  XOD_CUDA(cudaMemcpyAsync(dndt, dd, ns * pitch, cudaMemcpyDeviceToHost, s));
+  XOD_CUDA(cudaStreamSynchronize(s));
+  return XOD_OK;
+}
+
+xod_status xod_probe_fp64_peak(int cuda_device, int32_t iters, double *dfma_per_second) {
+  if (!dfma_per_second || iters <= 0) return fail(XOD_ERR_INVALID_ARG, "bad probe arguments");
+  XOD_CUDA(cudaSetDevice(cuda_device));
+  cudaDeviceProp prop;
+  XOD_CUDA(cudaGetDeviceProperties(&prop, cuda_device));
+  const int blocks = prop.multiProcessorCount * 8, threads = 256, inner = 4096;
+  double *out = nullptr;
+  XOD_CUDA(cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)));
+  cudaEvent_t e0, e1;
+  XOD_CUDA(cudaEventCreate(&e0));
+  XOD_CUDA(cudaEventCreate(&e1));
+  k_probe_dfma<<<blocks, threads>>>(out, inner, 1.0000001, 0.9999999);  // warm-up
+  XOD_CUDA(cudaEventRecord(e0));
+  for (int i = 0; i < iters; ++i) k_probe_dfma<<<blocks, threads>>>(out, inner, 1.0000001, 0.9999999);
+  XOD_CUDA(cudaEventRecord(e1));
+  XOD_CUDA(cudaEventSynchronize(e1));
+  float ms = 0;
+  XOD_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(out);
+  XOD_CUDA(cudaGetLastError());
+  *dfma_per_second = (double)blocks * threads * 16.0 * inner * iters / (ms * 1e-3);
+  return XOD_OK;
+}
+
+}  // extern "C"

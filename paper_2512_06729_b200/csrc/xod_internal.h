@@ -1,0 +1,92 @@
+// xod_internal.h -- host/device tables shared by the packer, the API layer and the kernels.
+// Part of libxodiac (the CUDA product path).  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/xodiac.h"
+
+namespace xod {
+
+// One Jacobian term: coef * k[dir][rxn] * n[o1] * n[o2]   (o < 0: factor 1)
+// (SURVEY §7.3 "Jacobian as gather"; never divides by n_j.)
+struct JacTerm {
+  int32_t rk;   // user reaction index; bit 31 set = reverse direction (uses kr)
+  int32_t o1;   // other species or -1
+  int32_t o2;   // other species or -1
+  float coef;   // nu_ir * m_jr, signed (reverse terms negative); |coef| <= 9, exact in fp32
+};
+
+// One warp's share of a source-CSR row inside a CTA task (see pack.cpp: build_source_schedule)
+struct SrcSeg {
+  int32_t row;     // species index, or -1 for an idle warp slot
+  int32_t begin;   // first CSR entry
+  int32_t end;     // one past the last CSR entry
+  int32_t nseg;    // >0 on the FIRST segment of a row: number of segments to combine; 0 otherwise
+};
+
+constexpr int kSrcWarpsPerCta = 8;
+constexpr int kSrcSegMin = 48;  // rows up to this many entries are summed by a single warp
+
+// Device-side view (plain pointers, passed to kernels by value)
+struct DevTables {
+  int32_t ns, nr, n_photo;
+  int32_t uni_begin, bi_begin, fo_begin, ph_begin;  // packed ranges [uni_begin,bi_begin) ...
+  // per packed reaction
+  const double *c0, *c1, *c2;               // log2 A - beta log2 t_ref, beta, -gamma log2 e
+  const double *l0, *l1, *l2, *fcl, *cN;    // falloff extras, indexed by p - fo_begin
+  const int32_t *sp;                        // [nr][6] reactants r0 r1 r2, products p0 p1 p2 (-1 none)
+  const int32_t *flags;                     // bit0 reversible
+  const int32_t *user;                      // packed -> user reaction index
+  const int32_t *photo_row;                 // packed photolysis p - ph_begin -> row of J
+  // thermo
+  const double *nasa;                       // [ns][2][7] raw a1..a7 (lo, hi)
+  const double *nasa_l2;                    // [ns][2][7] pre-scaled for u_i = log2(e) G_i/RT (see k_thermo.cu)
+  const double *tmid;                       // [ns]
+  // source CSR (device copy uses packed reaction indices = rows of q)
+  const int32_t *src_rxn;                   // [nnz_source] packed index
+  const float *src_nu;                      // [nnz_source]
+  const SrcSeg *src_seg;                    // [n_src_tasks][kSrcWarpsPerCta]
+  int32_t n_src_tasks;
+  // Jacobian
+  const int64_t *jac_term_ptr;              // [nnz_jac + 1]
+  const JacTerm *jac_terms;
+  int64_t nnz_jac;
+};
+
+struct HostTables {
+  int32_t ns = 0, ne = 0, nr = 0, n_photo = 0;
+  int32_t uni_begin = 0, bi_begin = 0, fo_begin = 0, ph_begin = 0;
+  std::vector<int32_t> packed_to_user, user_to_packed, photo_user;
+  std::vector<double> c0, c1, c2, l0, l1, l2, fcl, cN;
+  std::vector<int32_t> sp, flags, photo_row;
+  std::vector<double> nasa, nasa_l2, tmid;
+  // user-facing CSRs
+  std::vector<int64_t> src_ptr;
+  std::vector<int32_t> src_rxn_user, src_nu;
+  std::vector<int64_t> jac_ptr;
+  std::vector<int32_t> jac_col;
+  // device-facing
+  std::vector<int32_t> src_rxn_packed;
+  std::vector<float> src_nu_f;
+  std::vector<SrcSeg> src_seg;
+  std::vector<int64_t> jac_term_ptr;
+  std::vector<JacTerm> jac_terms;
+};
+
+// pack.cpp
+xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &err);
+
+}  // namespace xod
+
+struct xod_network {
+  xod::HostTables h;
+  xod::DevTables d{};
+  int device = -1;
+  std::vector<void *> dev_allocs;
+  int64_t chunk_cols = 0;  // 0 = default
+  // staging for the *_host call
+  void *stage = nullptr;
+  size_t stage_bytes = 0;
+};
