@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the XODIAC chemical source term on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload config4]
+
+One step = one pass of the hot path a1-a8 (thermo -> k_f -> k_r -> rates -> dn/dt, the metric's
+"rate + dn/dt") over one batch of synthetic columns through the C ABI call xod_source_fused.
+Workload at N = 1: BASELINE.json config 4 (594 species, 7 720 reactions, 256 atmospheres x 150
+layers = 38 400 columns, 2.96e8 (layer x reaction) evaluations per step).  N > 1: independent
+replicas of the same batch, one per GPU, no collective on the data path ("replicas only").
+Prints ONE JSON line (rank 0).  `stages` in that line carries the other calls of the boundary
+(xod_thermo, xod_rate_coeffs, xod_source, xod_jacobian on config 5, config 3 latency).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 rate+dn/dt evals/s (layer*reaction) at 7720 rxn"
+UNIT = "evals/s"
+# Algorithmic FP64-pipe instructions per evaluation of the fused path:
+# what the method must compute per (column, reaction), counted as FP64 instructions, FMA = 1.
+ALG_FP64_INSTR_PER_EVAL = 65.0
+NOMINAL_DFMA_PER_S = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x clocks.max.sm
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config4", choices=["config3", "config4", "config5"])
+    ap.add_argument("--no-stages", action="store_true", help="skip the per-call stage timings")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload(name):
+    from paper_2512_06729_b200 import synth
+    cfg = int(name[-1])
+    net = synth.config_network(cfg)
+    atm = synth.config_atmosphere(cfg, net)
+    return cfg, net, atm
+
+
+# --------------------------------------------------------------------------- clocks during the timed region
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for _, r in self.rows]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm = sorted(float(r[0]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for k, nm in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(rows[0][1]), "reasons": reasons,
+                "power_w_max": max(float(r[2]) for r in rows), "samples": len(rows)}
+
+
+# --------------------------------------------------------------------------- the CPU oracle legs
+def oracle_throughput(net, atm_full, n_layers, target_s=10.0):
+    """The oracle as it stands (pure-fp64 build, one thread) on a bounded sample of the workload:
+    whole atmospheres from the front of the batch, as many as fit in about `target_s` seconds."""
+    from oracle import Oracle
+    orc = Oracle(extended=False)
+    nr = net.n_reactions
+
+    def run(ncol):
+        T, P = atm_full.T[:ncol].copy(), atm_full.P[:ncol].copy()
+        J, n = atm_full.J[:, :ncol].copy(), atm_full.n[:, :ncol].copy()
+        t0 = time.perf_counter()
+        orc.source_from_state(net, T, P, J, n, ncol)
+        return time.perf_counter() - t0
+
+    ncol = min(n_layers, atm_full.ncol)
+    dt = run(ncol)
+    want = int(max(1, min(atm_full.ncol // n_layers, target_s / max(dt, 1e-6))))
+    if want > 1:
+        ncol = want * n_layers
+        dt = run(ncol)
+    return {"value": ncol * nr / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "first %d of %d columns (%d atmospheres) of the workload, oracle fp64 build, gcc -O2, "
+                      "1 thread, %.2f s" % (ncol, atm_full.ncol, ncol // n_layers, dt)}, dt, ncol
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, net, atm = workload(args.workload)
+    n_layers = atm.meta["n_layers"]
+    per_step = 8.0 if args.steps + args.warmup <= 6 else max(1.0, 60.0 / (args.steps + args.warmup))
+    base, dt0, ncol = oracle_throughput(net, atm, n_layers, target_s=per_step)
+    from oracle import Oracle
+    orc = Oracle(extended=False)
+    T, P = atm.T[:ncol].copy(), atm.P[:ncol].copy()
+    J, n = atm.J[:, :ncol].copy(), atm.n[:, :ncol].copy()
+    for _ in range(args.warmup):
+        orc.source_from_state(net, T, P, J, n, ncol)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.source_from_state(net, T, P, J, n, ncol)
+    dt = (time.perf_counter() - t0) / args.steps
+    value = ncol * net.n_reactions / dt
+    base["value"] = value
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "BASELINE.json config %d (%d species, %d reactions), bounded sample: %d columns per step"
+                               % (cfg, net.n_species, net.n_reactions, ncol)},
+        "cpu_baseline": base,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# --------------------------------------------------------------------------- our arm
+def event_time_ms(fn, reps, stream_sync):
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream_sync()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def stage_timings(binding, h3, net, dev, ws_for):
+    """Per-call device times of the other entry points (3 warm-ups, then event-timed repeats).
+    Evaluation counts: columns x 7 720 per call."""
+    import torch
+    from paper_2512_06729_b200 import synth
+    out = {}
+    sync = torch.cuda.synchronize
+    nr, ns = net.n_reactions, net.n_species
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")        # > 126 MB L2
+
+    def timed(fn, reps, flush_l2):
+        for _ in range(3):
+            fn()
+        if not flush_l2:
+            return event_time_ms(fn, reps, sync)
+        tot = 0.0
+        for _ in range(reps):
+            flush.fill_(1)
+            tot += event_time_ms(fn, 1, sync)
+        return tot / reps
+
+    for cfg, reps in ((3, 200), (5, 5)):
+        atm = synth.config_atmosphere(cfg, net)
+        ncol, ld = atm.ncol, atm.ld
+        T, P, J, n = dev(atm.T), dev(atm.P), dev(atm.J), dev(atm.n)
+        ws = ws_for(max(h3.source_fused_workspace_bytes(ncol), h3.source_workspace_bytes(ncol),
+                        h3.rate_coeffs_workspace_bytes(ncol)))
+        kf = torch.empty((nr, ld), dtype=torch.float64, device="cuda")
+        kr = torch.empty_like(kf)
+        d = torch.empty((ns, ld), dtype=torch.float64, device="cuda")
+        th = [torch.empty((ns, ld), dtype=torch.float64, device="cuda") for _ in range(4)]
+        big = cfg == 5
+        calls = {
+            "thermo": lambda: h3.thermo(ncol, ld, T, *th),
+            "rate_coeffs": lambda: h3.rate_coeffs(ncol, ld, T, P, J, kf, kr, ws),
+            "source": lambda: h3.source(ncol, ld, kf, kr, n, d, workspace=ws),
+            "source_fused": lambda: h3.source_fused(ncol, ld, T, P, J, n, d, workspace=ws),
+        }
+        if big:
+            jac = torch.empty((h3.nnz_jac, ld), dtype=torch.float64, device="cuda")
+            calls["jacobian"] = lambda: h3.jacobian(ncol, ld, kf, kr, n, jac)
+        res = {"ncol": ncol, "l2": "flushed between calls" if big else "warm (back-to-back calls, as a solver issues them)"}
+        for name, fn in calls.items():
+            ms = timed(fn, reps, big)
+            res[name + "_ms"] = ms
+            if name in ("rate_coeffs", "source", "source_fused"):
+                res[name + "_evals_per_s"] = ncol * nr / (ms * 1e-3)
+        if big:
+            res["jacobian_bytes"] = (2 * nr + ns + h3.nnz_jac) * ncol * 8
+            res["jacobian_gbs"] = res["jacobian_bytes"] / (res["jacobian_ms"] * 1e-3) / 1e9
+            res["rate_coeffs_gbs"] = 2 * nr * ncol * 8 / (res["rate_coeffs_ms"] * 1e-3) / 1e9
+            res["thermo_gbs"] = 4 * ns * ncol * 8 / (res["thermo_ms"] * 1e-3) / 1e9
+            del jac
+        out["config%d" % cfg] = res
+        del kf, kr, d, th
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    from paper_2512_06729_b200 import binding, build
+    build.build()
+    cfg, net, atm = workload(args.workload)
+    h = binding.Network(net, device=local)
+    ncol, ld, ns, nr = atm.ncol, atm.ld, net.n_species, net.n_reactions
+
+    def dev(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    T, P, J, n = dev(atm.T), dev(atm.P), dev(atm.J), dev(atm.n)
+    dndt = torch.empty((ns, ld), dtype=torch.float64, device="cuda")
+    ws = torch.empty(h.source_fused_workspace_bytes(ncol) // 8 + 64, dtype=torch.float64, device="cuda")
+    step = lambda: h.source_fused(ncol, ld, T, P, J, n, dndt, workspace=ws)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput: W warm-ups, then exactly K steps between two events
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    h.tune(binding.XOD_TUNE_TIMING, 1)
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    l0 = binding.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    w0 = time.time()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    w1 = time.time()
+    launches = binding.launch_count() - l0
+    ms_total = e0.elapsed_time(e1)
+    kt = h.timing_read()
+    h.tune(binding.XOD_TUNE_TIMING, 0)
+    clocks = sampler.stop(w0, w1)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    evals_per_step = ncol * nr * world
+    value = evals_per_step / (ms_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
+    hT, hP, hJ, hn = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (atm.T, atm.P, atm.J, atm.n)]
+    hd = torch.empty((ns, ld), dtype=torch.float64).pin_memory()
+    e2e_step = lambda: h.source_fused_host(ncol, ld, hT, hP, hJ, hn, hd)
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    k2 = max(3, min(args.steps, 10))
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(k2):
+        e2e_step()
+    e1.record()
+    barrier()
+    e2e_ms = max(e0.elapsed_time(e1), 0.0) / k2
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+    h2d = (2 + net.n_photo + ns) * ld * 8
+    d2h = ns * ld * 8
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+        return
+
+    # ---- roofline of the dominant kernel (the fused coefficient + rate-of-progress kernel)
+    dfma = binding.probe_fp64_peak(local, 10)
+    k_ms, k_n = kt["rates"]
+    k_avg_ms = k_ms / max(k_n, 1)
+    evals_per_launch = ncol * nr * args.steps / max(k_n, 1)
+    achieved = ALG_FP64_INSTR_PER_EVAL * evals_per_launch / (k_avg_ms * 1e-3) * 2 / 1e12   # TFLOP/s, FMA = 2
+    peak = dfma * 2 / 1e12
+    roofline = {"bound": "alu", "kernel": "k_rates (a3-a7: k_f, k_r, rates of progress)", "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": "fp64 DFMA probe measured in this run (xod_probe_fp64_peak); nominal %.1f TFLOP/s"
+                               % (NOMINAL_DFMA_PER_S * 2 / 1e12),
+                "alg_fp64_instr_per_eval": ALG_FP64_INSTR_PER_EVAL, "kernel_ms_avg": k_avg_ms, "kernel_launches": k_n,
+                "kernel_share_of_step": k_ms / ms_total,
+                "kernel_ms": {k: v[0] / args.steps for k, v in kt.items() if v[1]}}
+    stages = None
+    if not args.no_stages:
+        del hT, hP, hJ, hn, hd
+        stages = stage_timings(binding, h, net, dev, lambda b: torch.empty(b // 8 + 64, dtype=torch.float64, device="cuda"))
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu, _, _ = oracle_throughput(net, atm, atm.meta["n_layers"], target_s=10.0)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": "BASELINE.json config %d: %d species, %d reactions, %d atmospheres x %d layers = %d columns "
+                               "per GPU, xod_source_fused (a1-a8)" % (cfg, ns, nr, atm.meta["n_atm"], atm.meta["n_layers"], ncol),
+                   "evals_per_step": evals_per_step, "parallelism": "replicas only (no collective)" if world > 1 else "1 GPU",
+                   "l2": "inputs larger than L2 (n and dn/dt are %.0f MB each per step)" % (ns * ld * 8 / 1e6)},
+        "clocks": clocks,
+        "e2e": {"value": evals_per_step / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "call": "xod_source_fused_host (pinned host buffers; H2D, kernels, D2H and sync inside the timed region)"},
+        "gpu_launches": launches,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    if stages:
+        line["stages"] = stages
+    print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -101,8 +101,20 @@ xod_status xod_network_source_csr(const xod_network *net, int64_t *row_ptr, int3
 xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int32_t *col);
 
 /* ---- tuning knobs (optional; defaults are chosen for B200) */
-enum { XOD_TUNE_CHUNK_COLS = 0 /* columns per pipeline chunk of the fused source call */ };
+enum {
+  XOD_TUNE_CHUNK_COLS = 0, /* columns per pipeline chunk of the fused source call (0 = default) */
+  XOD_TUNE_TIMING = 1      /* != 0: bracket every kernel launch with a CUDA event pair (measurement) */
+};
 xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
+
+/* ---- measurement: per-kernel device time of the launches made since the last read while
+ * XOD_TUNE_TIMING was on.  ms, launches: [XOD_KERNEL_COUNT], indexed by XOD_KERNEL_*; either may
+ * be NULL.  Synchronises on the last recorded event, then clears the record. */
+enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD_KERNEL_RATES_FROM_K = 3,
+       XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_COUNT = 6 };
+xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
+/* kernels launched by this library in this process so far (all networks, all threads) */
+int64_t xod_launch_count(void);
 
 /* ---- a2: NASA-7 thermochemistry.  T [ld]; each output [n_species][ld], any may be NULL. */
 xod_status xod_thermo(const xod_network *net, int64_t ncol, int64_t ld, const double *T,

@@ -15,7 +15,8 @@ _lib = None
 XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK = 1
-XOD_TUNE_CHUNK_COLS = 0
+XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING = 0, 1
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -24,7 +25,7 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_network_jac_pattern", "xod_network_tune", "xod_thermo",
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
-           "xod_source_fused_host", "xod_probe_fp64_peak"]
+           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count"]
 
 
 class XodError(RuntimeError):
@@ -55,6 +56,7 @@ def lib():
                      "xod_source_fused_workspace_bytes"):
             getattr(L, name).restype = C.c_size_t
             getattr(L, name).argtypes = [C.c_void_p, C.c_int64]
+        L.xod_launch_count.restype = C.c_int64
         L.xod_network_destroy.restype = None
         L.xod_network_destroy.argtypes = [C.c_void_p]
         _lib = L
@@ -148,6 +150,13 @@ class Network:
     def tune(self, knob, value):
         _check(lib().xod_network_tune(self._h, C.c_int32(knob), C.c_int64(value)))
 
+    def timing_read(self):
+        """{kernel name: (total ms, launches)} since the last read (XOD_TUNE_TIMING on)."""
+        ms = (C.c_double * len(KERNEL_NAMES))()
+        cnt = (C.c_int64 * len(KERNEL_NAMES))()
+        _check(lib().xod_network_timing_read(self._h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(KERNEL_NAMES)}
+
     # ---- workspace sizes
     def rate_coeffs_workspace_bytes(self, ncol):
         return lib().xod_rate_coeffs_workspace_bytes(self._h, ncol)
@@ -197,6 +206,10 @@ class Network:
             return C.c_void_p(a.data_ptr())
         _check(lib().xod_source_fused_host(self._h, C.c_int64(ncol), C.c_int64(ld), hp(T), hp(P), hp(J),
                                            hp(n), hp(dndt)))
+
+
+def launch_count():
+    return lib().xod_launch_count()
 
 
 def probe_fp64_peak(device=0, iters=20):

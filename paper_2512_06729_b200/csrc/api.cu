@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/xodiac.h: argument checks, workspace carving, kernel launches
 // on the caller's stream.  No host synchronisation in any compute call except *_host.
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -29,6 +30,32 @@ xod_status cuda_fail(cudaError_t e, const char *where) {
   } while (0)
 
 inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+std::atomic<int64_t> g_launches{0};  // kernels launched by this library in this process
+
+// Counts the launch and, when timing is on, brackets it with a CUDA event pair on the stream.
+struct Timed {
+  TimingState *t = nullptr;
+  cudaStream_t s;
+  size_t pair = 0;
+  Timed(const xod_network *net, int kid, cudaStream_t stream) : s(stream) {
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if (!net->timing.on) return;
+    t = &net->timing;
+    while (t->pool.size() < t->used + 2) {
+      cudaEvent_t e = nullptr;
+      if (cudaEventCreate(&e) != cudaSuccess) { t = nullptr; return; }
+      t->pool.push_back(e);
+    }
+    pair = t->used;
+    t->used += 2;
+    t->kid.push_back(kid);
+    cudaEventRecord(static_cast<cudaEvent_t>(t->pool[pair]), s);
+  }
+  ~Timed() {
+    if (t) cudaEventRecord(static_cast<cudaEvent_t>(t->pool[pair + 1]), s);
+  }
+};
 
 template <class T>
 xod_status upload(xod_network *net, const std::vector<T> &v, const T **dst) {
@@ -155,6 +182,7 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
 
 void xod_network_destroy(xod_network *net) {
   if (!net) return;
+  for (void *e : net->timing.pool) cudaEventDestroy(static_cast<cudaEvent_t>(e));
   for (void *p : net->dev_allocs) cudaFree(p);
   if (net->stage) cudaFree(net->stage);
   delete net;
@@ -209,6 +237,10 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
     net->chunk_cols = value;
     return XOD_OK;
   }
+  if (knob == XOD_TUNE_TIMING) {
+    net->timing.on = value != 0;
+    return XOD_OK;
+  }
   return fail(XOD_ERR_INVALID_ARG, "unknown tuning knob");
 }
 
@@ -227,7 +259,10 @@ xod_status xod_thermo(const xod_network *net, int64_t ncol, int64_t ld, const do
   int spb = net->h.ns;
   while (spb > 4 && gx * ((net->h.ns + spb - 1) / spb) < 148 * 8) spb = (spb + 1) / 2;
   dim3 grid((unsigned)gx, (unsigned)((net->h.ns + spb - 1) / spb));
-  k_thermo<<<grid, 128, 0, s>>>(net->d, ncol, ld, T, cp_R, h_RT, s_R, g_RT, spb);
+  {
+    Timed tm(net, KID_THERMO, s);
+    k_thermo<<<grid, 128, 0, s>>>(net->d, ncol, ld, T, cp_R, h_RT, s_R, g_RT, spb);
+  }
   XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
@@ -246,7 +281,10 @@ xod_status launch_prologue(const xod_network *net, int64_t ncol, int64_t col0, i
   int split = 1;
   while (split < 64 && ncg * split < 148 * 2 && split * 8 < net->h.ns) split *= 2;
   dim3 grid((unsigned)ncg, (unsigned)split);
-  k_prologue<<<grid, 256, 0, s>>>(net->d, ncol, col0, T, P, w, kLog2Kb);
+  {
+    Timed tm(net, KID_PROLOGUE, s);
+    k_prologue<<<grid, 256, 0, s>>>(net->d, ncol, col0, T, P, w, kLog2Kb);
+  }
   XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
@@ -259,7 +297,10 @@ xod_status launch_rates(const xod_network *net, int64_t ncol, int64_t col0, int6
   const int64_t nslices = (net->h.nr + rw - 1) / rw;
   const int64_t ntasks = nslices * ncg;
   const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, 148LL * 16);
-  k_rates<MODE><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, J, n, kf, kr, rw, (int)ncg, ntasks);
+  {
+    Timed tm(net, KID_RATES, s);
+    k_rates<MODE><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, J, n, kf, kr, rw, (int)ncg, ntasks);
+  }
   XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
@@ -268,7 +309,10 @@ template <bool PL>
 xod_status launch_source(const xod_network *net, int64_t ncol, int64_t col0, int64_t ld, int64_t ncg,
                          const ChunkScratch &w, double *dndt, double *prod, double *loss, cudaStream_t s) {
   dim3 grid((unsigned)net->d.n_src_tasks, (unsigned)ncg);
-  k_source<PL><<<grid, 256, 0, s>>>(net->d, ncol, col0, ld, w, dndt, prod, loss);
+  {
+    Timed tm(net, KID_SOURCE, s);
+    k_source<PL><<<grid, 256, 0, s>>>(net->d, ncol, col0, ld, w, dndt, prod, loss);
+  }
   XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
@@ -325,6 +369,7 @@ xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const do
       const int rw = pick_rw(net->h.nr, ncg);
       const int64_t ntasks = (int64_t)((net->h.nr + rw - 1) / rw) * ncg;
       const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, 148LL * 16);
+      Timed tm(net, KID_RATES_FROM_K, s);
       if (pl)
         k_rates_from_k<MODE_QSEP><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, kf, kr, n, rw, (int)ncg, ntasks);
       else
@@ -387,7 +432,10 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
   const int64_t want = (net->d.nnz_jac + 7) / 8;
   const int64_t gx = std::max<int64_t>(1, std::min<int64_t>(want, std::max<int64_t>(1, 148LL * 64 / ncg)));
   dim3 grid((unsigned)gx, (unsigned)ncg);
-  k_jacobian<<<grid, 256, 0, s>>>(net->d, ncol, ld, kf, kr, n, jac);
+  {
+    Timed tm(net, KID_JACOBIAN, s);
+    k_jacobian<<<grid, 256, 0, s>>>(net->d, ncol, ld, kf, kr, n, jac);
+  }
   XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
@@ -422,6 +470,27 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
   if (st != XOD_OK) return st;
   XOD_CUDA(cudaMemcpyAsync(dndt, dd, ns * pitch, cudaMemcpyDeviceToHost, s));
   XOD_CUDA(cudaStreamSynchronize(s));
+  return XOD_OK;
+}
+
+int64_t xod_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  TimingState &t = net->timing;
+  for (int k = 0; k < KID_COUNT; ++k) {
+    if (ms) ms[k] = 0;
+    if (launches) launches[k] = 0;
+  }
+  if (t.used) XOD_CUDA(cudaEventSynchronize(static_cast<cudaEvent_t>(t.pool[t.used - 1])));
+  for (size_t p = 0; p < t.kid.size(); ++p) {
+    float f = 0;
+    XOD_CUDA(cudaEventElapsedTime(&f, static_cast<cudaEvent_t>(t.pool[2 * p]), static_cast<cudaEvent_t>(t.pool[2 * p + 1])));
+    if (ms) ms[t.kid[p]] += f;
+    if (launches) ++launches[t.kid[p]];
+  }
+  t.used = 0;
+  t.kid.clear();
   return XOD_OK;
 }
 

@@ -80,6 +80,18 @@ xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &e
 
 }  // namespace xod
 
+// optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
+// every launch on the caller's stream, summed by xod_network_timing_read
+namespace xod {
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_COUNT };
+struct TimingState {
+  bool on = false;
+  std::vector<void *> pool;                       // cudaEvent_t, reused
+  size_t used = 0;
+  std::vector<int> kid;                           // kernel id of pair p = events 2p, 2p+1
+};
+}  // namespace xod
+
 struct xod_network {
   xod::HostTables h;
   xod::DevTables d{};
@@ -89,4 +101,5 @@ struct xod_network {
   // staging for the *_host call
   void *stage = nullptr;
   size_t stage_bytes = 0;
+  mutable xod::TimingState timing;
 };

@@ -1,0 +1,62 @@
+"""Helpers of the `-m gpu` parity tests: device buffers, the tolerance rules of BASELINE.json
+north_star and DESIGN.md reading R5.  Marshalling and comparison only; no method arithmetic."""
+import numpy as np
+
+TOL_K = 1e-12        # k_f, k_r: relative (north_star)
+TOL_SUM = 1e-11      # dn/dt and Jacobian: of sum |contributing terms| per entry (north_star)
+TOL_THERMO = 1e-13   # thermo: of sum |polynomial terms| (derived from the arithmetic)
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).cuda()
+
+
+def empty(rows, ld, fill=np.nan):
+    import torch
+    return torch.full((rows, ld), fill, dtype=torch.float64, device="cuda")
+
+
+def workspace(nbytes):
+    import torch
+    return torch.empty((nbytes + 7) // 8 + 32, dtype=torch.float64, device="cuda")
+
+
+def host(t):
+    import torch
+    torch.cuda.synchronize()
+    return t.cpu().numpy()
+
+
+def check_k(got, want, what):
+    """Reading R5: oracle inf -> GPU inf; oracle 0 or subnormal -> |GPU| <= 1e-300; else rel 1e-12."""
+    want_inf = np.isinf(want)
+    assert np.array_equal(np.isinf(got), want_inf), "%s: inf pattern differs" % what
+    tiny = np.abs(want) < 2.2250738585072014e-308
+    assert np.all(np.abs(got[tiny]) <= 1e-300), "%s: oracle underflow but GPU not tiny" % what
+    m = ~want_inf & ~tiny
+    rel = np.abs(got[m] - want[m]) / np.abs(want[m])
+    worst = float(rel.max()) if rel.size else 0.0
+    assert worst <= TOL_K, "%s: max relative error %.3e > %.0e" % (what, worst, TOL_K)
+    return worst
+
+
+def finite_columns(*arrays):
+    """Columns on which every entry of every array is finite (reading R5: dn/dt, Jacobian and
+    conservation are compared only there)."""
+    ok = None
+    for a in arrays:
+        f = np.all(np.isfinite(a), axis=0)
+        ok = f if ok is None else ok & f
+    return ok
+
+
+def check_sum(got, want, scale, cols, what, tol=TOL_SUM):
+    """|got - want| <= tol * scale on the given columns; scale == 0 demands exact equality."""
+    g, w, s = got[:, cols], want[:, cols], scale[:, cols]
+    err = np.abs(g - w)
+    bad = err > tol * s
+    assert not bad.any(), "%s: %d entries beyond %.0e x scale (worst ratio %.3e)" % (
+        what, int(bad.sum()), tol, float((err[bad] / np.maximum(s[bad], 1e-300)).max()))
+    nz = s > 0
+    return float((err[nz] / s[nz]).max()) if nz.any() else 0.0

@@ -1,0 +1,329 @@
+"""`-m gpu` parity tests: the CUDA path, called through the C ABI (paper_2512_06729_b200.binding),
+against the CPU oracle on the same seeded inputs, element by element.
+
+Tolerances (BASELINE.json north_star): k_f, k_r relative 1e-12; dn/dt and Jacobian entries 1e-11
+of sum |contributing terms| per entry; CSR layouts bit-exact (tests/test_boundary.py).  Thermo:
+1e-13 of sum |polynomial terms|.  Overflow rule: DESIGN.md reading R5."""
+import numpy as np
+import pytest
+
+import gpu_common as G
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def xod():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the gpu tests need the B200 box (there is no CPU fallback)")
+    from paper_2512_06729_b200 import binding, build
+    build.build()
+    binding.lib()
+    return binding
+
+
+_handles = {}
+
+
+def handle(xod, network, cfg):
+    key = 3 if cfg in (3, 4, 5) else cfg
+    if key not in _handles:
+        _handles[key] = xod.Network(network(key), device=0)
+    return _handles[key]
+
+
+def atmosphere(cfg, net, n_atm=None):
+    from paper_2512_06729_b200 import synth
+    return synth.config_atmosphere(cfg, net, n_atm)
+
+
+def thermo_scale(net, T):
+    """sum |terms| of each NASA-7 form (tolerance scale only)."""
+    T = np.asarray(T)[None, :]
+    a = np.where((T <= net.t_mid[:, None])[:, :, None], net.nasa_lo[:, None, :], net.nasa_hi[:, None, :])
+    a = np.abs(a)
+    lnT = np.abs(np.log(T))
+    p = [a[:, :, k] * T ** k for k in range(5)]
+    cp = sum(p)
+    h = p[0] + p[1] / 2 + p[2] / 3 + p[3] / 4 + p[4] / 5 + a[:, :, 5] / T
+    s = a[:, :, 0] * lnT + p[1] + p[2] / 2 + p[3] / 3 + p[4] / 4 + a[:, :, 6]
+    g = a[:, :, 0] * (1 + lnT) + p[1] / 2 + p[2] / 6 + p[3] / 12 + p[4] / 20 + a[:, :, 5] / T + a[:, :, 6]
+    return cp, h, s, g
+
+
+# ------------------------------------------------------------------------------- a2 thermo
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_thermo_matches_oracle(xod, oracle, network, cfg):
+    net = network(cfg)
+    h = handle(xod, network, cfg)
+    atm = atmosphere(cfg, net)
+    want = oracle.thermo(net, atm.T, atm.ncol)
+    outs = [G.empty(net.n_species, atm.ld) for _ in range(4)]
+    h.thermo(atm.ncol, atm.ld, G.dev(atm.T), *outs)
+    scales = thermo_scale(net, atm.T)
+    c = slice(0, atm.ncol)
+    for name, got, w, s in zip(("cp/R", "H/RT", "S/R", "G/RT"), outs, want, scales):
+        got = G.host(got)
+        assert np.all(np.abs(got[:, c] - w[:, c]) <= G.TOL_THERMO * s[:, c]), name
+        assert np.all(np.isnan(got[:, atm.ncol:])), "%s: padding columns were written" % name
+    # optional outputs: only G/RT requested
+    g_only = G.empty(net.n_species, atm.ld)
+    h.thermo(atm.ncol, atm.ld, G.dev(atm.T), None, None, None, g_only)
+    assert np.array_equal(G.host(g_only)[:, c], G.host(outs[3])[:, c])
+
+
+def test_thermo_range_selection_at_t_mid(xod, oracle, network):
+    """Reading T3: T <= t_mid -> low set; exactly t_mid -> low."""
+    net = network(2)
+    h = handle(xod, network, 2)
+    tm = float(net.t_mid[0])
+    T = np.array([np.nextafter(tm, 0), tm, np.nextafter(tm, 1e9), 300.0, 500.0, 700.0, 1000.0, 150.0, 6000.0])
+    want = oracle.thermo(net, T)
+    outs = [G.empty(net.n_species, T.size) for _ in range(4)]
+    h.thermo(T.size, T.size, G.dev(T), *outs)
+    for got, w, s in zip(outs, want, thermo_scale(net, T)):
+        assert np.all(np.abs(G.host(got) - w) <= G.TOL_THERMO * s)
+
+
+# ------------------------------------------------------------------------------- a1, a3-a6 coefficients
+def run_rate_coeffs(h, atm, ncol=None, ld=None):
+    ncol = atm.ncol if ncol is None else ncol
+    ld = atm.ld if ld is None else ld
+    kf, kr = G.empty(h.n_reactions, ld), G.empty(h.n_reactions, ld)
+    ws = G.workspace(h.rate_coeffs_workspace_bytes(ncol))
+    h.rate_coeffs(ncol, ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), kf, kr, ws)
+    return G.host(kf), G.host(kr)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_rate_coeffs_match_oracle(xod, oracle, network, cfg):
+    net = network(cfg)
+    h = handle(xod, network, cfg)
+    atm = atmosphere(cfg, net)
+    kf, kr = run_rate_coeffs(h, atm)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    c = slice(0, atm.ncol)
+    G.check_k(kf[:, c], okf[:, c], "k_f config %d" % cfg)
+    G.check_k(kr[:, c], okr[:, c], "k_r config %d" % cfg)
+    assert np.all(np.isnan(kf[:, atm.ncol:])) and np.all(np.isnan(kr[:, atm.ncol:]))
+    photo = net.type == 3
+    assert np.array_equal(kf[photo][:, c], atm.J[:, c])           # a5: k_f = J bit for bit
+    assert np.all(kr[photo][:, c] == 0.0)
+
+
+def test_rate_coeffs_cold_columns_overflow_rule(xod, oracle, network):
+    """Config 4's cold T shifts drive |dG/RT| past the double range (reading R5): inf where the
+    oracle (long double, rounded at the end) is inf, tiny where it underflows, 1e-12 elsewhere."""
+    net = network(4)
+    h = handle(xod, network, 4)
+    atm = atmosphere(4, net, n_atm=6)
+    assert atm.T[:atm.ncol].min() < 450.0
+    kf, kr = run_rate_coeffs(h, atm)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    c = slice(0, atm.ncol)
+    G.check_k(kf[:, c], okf[:, c], "k_f config 4")
+    G.check_k(kr[:, c], okr[:, c], "k_r config 4")
+    assert np.isinf(okr[:, c]).any(), "the sample was meant to contain overflowing k_r"
+
+
+def test_kooij_reference_temperature(xod, oracle, network):
+    """Reading K1: t_ref = 300 (Kooij) on some reactions."""
+    import copy
+    net = copy.copy(network(1))
+    net.t_ref = np.where(np.arange(net.n_reactions) % 2 == 0, 300.0, 1.0)
+    h = xod.Network(net, device=0)
+    atm = atmosphere(1, net)
+    kf, kr = run_rate_coeffs(h, atm)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    G.check_k(kf[:, :atm.ncol], okf[:, :atm.ncol], "k_f Kooij")
+    G.check_k(kr[:, :atm.ncol], okr[:, :atm.ncol], "k_r Kooij")
+    h.close()
+
+
+# ------------------------------------------------------------------------------- a7-a8 source
+def element_residual(net, dndt, scale, cols):
+    """max over (element, column) of |sum_i a_ie dn_i/dt| / sum_i |a_ie| S_i."""
+    a = net.composition.astype(np.float64)
+    num = np.abs(a.T @ dndt[:, cols])
+    den = np.abs(a).T @ scale[:, cols]
+    m = den > 0
+    return float((num[m] / den[m]).max())
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_source_from_stored_coefficients(xod, oracle, network, cfg):
+    net = network(cfg)
+    h = handle(xod, network, cfg)
+    atm = atmosphere(cfg, net)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    ns, ld = net.n_species, atm.ld
+    ws = G.workspace(h.source_workspace_bytes(atm.ncol))
+    d0 = G.empty(ns, ld)
+    h.source(atm.ncol, ld, G.dev(okf), G.dev(okr), G.dev(atm.n), d0, workspace=ws)
+    d1, p1, l1 = G.empty(ns, ld), G.empty(ns, ld), G.empty(ns, ld)
+    h.source(atm.ncol, ld, G.dev(okf), G.dev(okr), G.dev(atm.n), d1, p1, l1, workspace=ws)
+    cols = np.arange(atm.ncol)
+    scale = wp + wl
+    for got in (G.host(d0), G.host(d1)):
+        G.check_sum(got, want, scale, cols, "dn/dt config %d" % cfg)
+        assert np.all(np.isnan(got[:, atm.ncol:]))
+        assert element_residual(net, got, scale, cols) <= 1e-13
+    G.check_sum(G.host(p1), wp, scale, cols, "P")
+    G.check_sum(G.host(l1), wl, scale, cols, "L")
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_source_fused_matches_oracle(xod, oracle, network, cfg):
+    """The headline path a1-a8: (T, P, J, n) -> dn/dt with k_f, k_r never stored."""
+    net = network(cfg)
+    h = handle(xod, network, cfg)
+    atm = atmosphere(cfg, net)
+    want, wp, wl = oracle.source_from_state(net, atm.T, atm.P, atm.J, atm.n, atm.ncol)
+    ns, ld = net.n_species, atm.ld
+    ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+    d0 = G.empty(ns, ld)
+    h.source_fused(atm.ncol, ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    d1, p1, l1 = G.empty(ns, ld), G.empty(ns, ld), G.empty(ns, ld)
+    h.source_fused(atm.ncol, ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d1, p1, l1,
+                   workspace=ws)
+    cols = np.arange(atm.ncol)
+    scale = wp + wl
+    for got in (G.host(d0), G.host(d1)):
+        G.check_sum(got, want, scale, cols, "fused dn/dt config %d" % cfg)
+        assert np.all(np.isnan(got[:, atm.ncol:]))
+        assert element_residual(net, got, scale, cols) <= 1e-13
+    G.check_sum(G.host(p1), wp, scale, cols, "fused P")
+    G.check_sum(G.host(l1), wl, scale, cols, "fused L")
+    # the host-buffer entry point runs the same kernels
+    out = np.full((ns, ld), np.nan)
+    h.source_fused_host(atm.ncol, ld, atm.T, atm.P, atm.J, atm.n, out)
+    assert np.array_equal(out[:, :atm.ncol], G.host(d0)[:, :atm.ncol])
+
+
+def test_source_fused_config4_batch(xod, oracle, network):
+    """Config 4 family (T shifts, metallicity): several chunks, a ragged tail, and columns with
+    non-finite k_r excluded by reading R5 (their count is reported, and must be > 0 here)."""
+    net = network(4)
+    h = handle(xod, network, 4)
+    atm = atmosphere(4, net, n_atm=9)                 # 1350 columns: 2 chunks of 1024, ragged
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    ns, ld = net.n_species, atm.ld
+    ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+    d0 = G.empty(ns, ld)
+    h.source_fused(atm.ncol, ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    ok = G.finite_columns(okf[:, :atm.ncol], okr[:, :atm.ncol], want[:, :atm.ncol], wp[:, :atm.ncol], wl[:, :atm.ncol])
+    cols = np.flatnonzero(ok)
+    excluded = atm.ncol - cols.size
+    print("config 4 sample: %d of %d columns excluded by R5" % (excluded, atm.ncol))
+    assert 0 < excluded < atm.ncol
+    got = G.host(d0)
+    scale = wp + wl
+    G.check_sum(got, want, scale, cols, "fused dn/dt config 4")
+    assert element_residual(net, got, scale, cols) <= 1e-13
+
+
+# ------------------------------------------------------------------------------- a9 Jacobian
+@pytest.mark.parametrize("cfg,n_atm", [(1, None), (2, None), (5, 1)])
+def test_jacobian_matches_oracle(xod, oracle, network, cfg, n_atm):
+    net = network(cfg)
+    h = handle(xod, network, cfg)
+    atm = atmosphere(cfg, net, n_atm)
+    ncol = atm.ncol if cfg != 5 else 40               # the dense oracle is O(ns^2) per column
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    rp, col = h.jac_pattern()
+    want, scale = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
+    jac = G.empty(h.nnz_jac, atm.ld)
+    h.jacobian(ncol, atm.ld, G.dev(okf), G.dev(okr), G.dev(atm.n), jac)
+    got = G.host(jac)
+    G.check_sum(got, want, scale, np.arange(ncol), "Jacobian config %d" % cfg)
+    assert np.all(np.isnan(got[:, ncol:]))
+    # element conservation of the Jacobian: sum_i a_ie Jac_ij = 0 for every (e, j)
+    rows = np.repeat(np.arange(net.n_species), np.diff(rp))
+    a = net.composition.astype(np.float64)
+    for e in range(net.n_elements):
+        num = np.zeros((net.n_species, ncol))
+        den = np.zeros((net.n_species, ncol))
+        np.add.at(num, col, a[rows, e][:, None] * got[:, :ncol])
+        np.add.at(den, col, np.abs(a[rows, e])[:, None] * scale[:, :ncol])
+        m = den > 0
+        assert np.all(np.abs(num[m]) <= 1e-13 * den[m])
+
+
+# ------------------------------------------------------------------------------- edge cases
+def test_zero_densities_give_exact_zeros(xod, oracle, network):
+    """Reading Q2: n = 0 is legal; the Jacobian never divides by n_j."""
+    net = network(2)
+    h = handle(xod, network, 2)
+    atm = atmosphere(2, net)
+    n = atm.n.copy()
+    n[::3, :] = 0.0
+    n[:, 5] = 0.0
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, n, atm.ncol)
+    ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+    d0 = G.empty(net.n_species, atm.ld)
+    h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(n), d0, workspace=ws)
+    got = G.host(d0)
+    G.check_sum(got, want, wp + wl, np.arange(atm.ncol), "dn/dt with zeros")
+    assert np.all(got[:, 5] == 0.0)
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, n, rp, col, atm.ncol)
+    jac = G.empty(h.nnz_jac, atm.ld)
+    h.jacobian(atm.ncol, atm.ld, G.dev(okf), G.dev(okr), G.dev(n), jac)
+    G.check_sum(G.host(jac), wj, sj, np.arange(atm.ncol), "Jacobian with zeros")
+
+
+@pytest.mark.parametrize("ncol,ld", [(0, 32), (1, 1), (31, 40), (33, 64), (150, 150), (97, 256)])
+def test_ragged_sizes_and_pitches(xod, oracle, network, ncol, ld):
+    """Empty, single-column, sub-warp, just-over-a-warp sizes and pitches that are not multiples
+    of 32; columns beyond ncol are never touched."""
+    from paper_2512_06729_b200 import synth
+    net = network(2)
+    h = handle(xod, network, 2)
+    atm = synth.make_atmosphere(77, net, 1, max(ncol, 1), ld=ld)
+    want, wp, wl = oracle.source_from_state(net, atm.T, atm.P, atm.J, atm.n, ncol)
+    ws = G.workspace(h.source_fused_workspace_bytes(ncol))
+    d0 = G.empty(net.n_species, ld)
+    h.source_fused(ncol, ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    got = G.host(d0)
+    G.check_sum(got, want, wp + wl, np.arange(ncol), "ragged dn/dt")
+    assert np.all(np.isnan(got[:, ncol:]))
+    kf, kr = run_rate_coeffs(h, atm, ncol, ld)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    G.check_k(kf[:, :ncol], okf[:, :ncol], "ragged k_f")
+    G.check_k(kr[:, :ncol], okr[:, :ncol], "ragged k_r")
+    assert np.all(np.isnan(kf[:, ncol:]))
+
+
+def test_chunk_boundaries_do_not_change_results(xod, network):
+    """The column-chunk pipeline must be invisible: 64-column chunks == one chunk, bit for bit."""
+    net = network(3)
+    atm = atmosphere(3, net)
+    outs = []
+    for chunk in (0, 64):
+        h = xod.Network(net, device=0)
+        h.tune(xod.XOD_TUNE_CHUNK_COLS, chunk)
+        ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+        d0 = G.empty(net.n_species, atm.ld)
+        h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+        outs.append(G.host(d0)[:, :atm.ncol])
+        h.close()
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_workspace_too_small_is_an_error(xod, network):
+    net = network(1)
+    h = handle(xod, network, 1)
+    atm = atmosphere(1, net)
+    d0 = G.empty(net.n_species, atm.ld)
+    with pytest.raises(xod.XodError) as e:
+        h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0,
+                       workspace=G.dev(np.zeros(4)))
+    assert e.value.status == 5
+    with pytest.raises(xod.XodError) as e:
+        h.source_fused(atm.ncol, atm.ncol - 1, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0,
+                       workspace=G.workspace(h.source_fused_workspace_bytes(atm.ncol)))
+    assert e.value.status == 1
