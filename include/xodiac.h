@@ -100,10 +100,17 @@ xod_status xod_network_source_csr(const xod_network *net, int64_t *row_ptr, int3
  * diagonal; rows = species, ascending column indices; row_ptr [n_species+1], col [nnz_jac] */
 xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int32_t *col);
 
+/* layout of the single-kernel fused path (xod_source_fused), info[10]: enabled, reactions per chunk,
+ * chunks, accumulator rows, thermo breakpoints, shared-memory bytes per CTA, padded reactions,
+ * production/loss warp tasks, padded production/loss entries, bytes of the reverse-coefficient table */
+xod_status xod_network_fused_info(const xod_network *net, int64_t *info);
+
 /* ---- tuning knobs (optional; defaults are chosen for B200) */
 enum {
   XOD_TUNE_CHUNK_COLS = 0, /* columns per pipeline chunk of the fused source call (0 = default) */
-  XOD_TUNE_TIMING = 1      /* != 0: bracket every kernel launch with a CUDA event pair (measurement) */
+  XOD_TUNE_TIMING = 1,     /* != 0: bracket every kernel launch with a CUDA event pair (measurement) */
+  XOD_TUNE_SPLIT = 2,      /* reaction splits per column tile of the single-kernel fused path (0 = auto) */
+  XOD_TUNE_FUSED_KERNEL = 3 /* 0: xod_source_fused uses the multi-kernel pipeline instead (default 1) */
 };
 xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
 
@@ -111,7 +118,8 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
  * XOD_TUNE_TIMING was on.  ms, launches: [XOD_KERNEL_COUNT], indexed by XOD_KERNEL_*; either may
  * be NULL.  Synchronises on the last recorded event, then clears the record. */
 enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD_KERNEL_RATES_FROM_K = 3,
-       XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_COUNT = 6 };
+       XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
+       XOD_KERNEL_COUNT = 8 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);

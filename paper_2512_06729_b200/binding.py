@@ -15,8 +15,8 @@ _lib = None
 XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK = 1
-XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING = 0, 1
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian"]
+XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL = 0, 1, 2, 3
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -25,7 +25,7 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_network_jac_pattern", "xod_network_tune", "xod_thermo",
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
-           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count"]
+           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info"]
 
 
 class XodError(RuntimeError):
@@ -146,6 +146,12 @@ class Network:
         col = np.zeros(self.nnz_jac, dtype=np.int32)
         _check(lib().xod_network_jac_pattern(self._h, _hp(rp), _hp(col)))
         return rp, col
+
+    def fused_info(self):
+        v = (C.c_int64 * 10)()
+        _check(lib().xod_network_fused_info(self._h, v))
+        keys = ("enabled", "chunk", "nchunk", "n_acc", "n_bp", "smem_bytes", "npad", "tasks", "entries", "rev_bytes")
+        return dict(zip(keys, [int(x) for x in v]))
 
     def tune(self, knob, value):
         _check(lib().xod_network_tune(self._h, C.c_int32(knob), C.c_int64(value)))

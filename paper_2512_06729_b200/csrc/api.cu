@@ -7,6 +7,7 @@
 #include <new>
 #include <string>
 
+#include "fused.cuh"
 #include "kernels.cuh"
 
 using namespace xod;
@@ -69,6 +70,7 @@ xod_status upload(xod_network *net, const std::vector<T> &v, const T **dst) {
 }
 
 const double kLog2Kb = (double)std::log2(1.380649e-16L);
+constexpr size_t kFusedSmemMax = 227 * 1024;  // shared memory one CTA may opt into on sm_100
 
 constexpr int64_t kDefaultChunk = 1024;  // columns per pipeline chunk: q chunk = nr*1024*8 B stays in L2
 
@@ -145,6 +147,17 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
     return fail(st, err);
   }
   net->device = cuda_device;
+  // tables of the single-kernel fused path: the largest chunk whose shared memory fits one CTA
+  try {
+    for (int chunk : {256, 192, 128, 64}) {
+      pack_fused(desc, net->h, chunk);
+      if (net->h.f.enabled && fused_smem_bytes(net->h.ns, net->h.f.n_acc, chunk) <= kFusedSmemMax) break;
+      net->h.f.enabled = false;
+    }
+  } catch (const std::bad_alloc &) {
+    delete net;
+    return fail(XOD_ERR_ALLOC, "out of host memory while packing");
+  }
   if (cuda_device >= 0) {
     int prev = -1;
     cudaError_t e = cudaGetDevice(&prev);
@@ -167,6 +180,27 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
     UP(nasa, nasa); UP(nasa_l2, nasa_l2); UP(tmid, tmid);
     UP(src_rxn_packed, src_rxn); UP(src_nu_f, src_nu); UP(src_seg, src_seg);
     UP(jac_term_ptr, jac_term_ptr); UP(jac_terms, jac_terms);
+    if (h.f.enabled) {
+      FusedHost &f = h.f;
+      FusedDev &fd = net->fd;
+      fd.enabled = 1;
+      fd.npad = f.npad, fd.arr_end = f.arr_end, fd.fo_end = f.fo_end, fd.ph_end = f.ph_end;
+      fd.chunk = f.chunk, fd.nchunk = f.nchunk, fd.n_acc = f.n_acc, fd.n_bp = f.n_bp;
+      fd.n_extra = (int32_t)(f.extra.size() / 2);
+#define UPF(vec, field) if (st == XOD_OK) st = upload(net, f.vec, &fd.field)
+      UPF(bp, bp); UPF(c, c); UPF(l, l); UPF(rev, rev); UPF(sp, sp); UPF(task_ptr, task_ptr);
+      UPF(task, task); UPF(entry, entry); UPF(extra, extra);
+#undef UPF
+      if (st == XOD_OK) {
+        // the attribute is per function, not per network: always opt into the device maximum
+        cudaError_t ce = cudaFuncSetAttribute(k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                              (int)kFusedSmemMax);
+        if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_fused)");
+      }
+      int smc = 0;
+      if (cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, cuda_device) == cudaSuccess && smc > 0)
+        net->sm_count = smc;
+    }
 #undef UP
     if (prev >= 0 && prev != cuda_device) cudaSetDevice(prev);
     if (st != XOD_OK) {
@@ -230,11 +264,30 @@ xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int
   return XOD_OK;
 }
 
+xod_status xod_network_fused_info(const xod_network *net, int64_t *info) {
+  if (!net || !info) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
+  const FusedHost &f = net->h.f;
+  info[0] = f.enabled, info[1] = f.chunk, info[2] = f.nchunk, info[3] = f.n_acc, info[4] = f.n_bp;
+  info[5] = f.enabled ? (int64_t)fused_smem_bytes(net->h.ns, f.n_acc, f.chunk) : 0;
+  info[6] = f.npad, info[7] = (int64_t)f.task.size(), info[8] = (int64_t)f.entry.size();
+  info[9] = (int64_t)(f.rev.size() * sizeof(double));
+  return XOD_OK;
+}
+
 xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
   if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
   if (knob == XOD_TUNE_CHUNK_COLS) {
     if (value < 0) return fail(XOD_ERR_INVALID_ARG, "chunk columns must be >= 0");
     net->chunk_cols = value;
+    return XOD_OK;
+  }
+  if (knob == XOD_TUNE_SPLIT) {
+    if (value < 0) return fail(XOD_ERR_INVALID_ARG, "split must be >= 0");
+    net->force_split = value;
+    return XOD_OK;
+  }
+  if (knob == XOD_TUNE_FUSED_KERNEL) {
+    net->use_fused = value;
     return XOD_OK;
   }
   if (knob == XOD_TUNE_TIMING) {
@@ -300,6 +353,41 @@ xod_status launch_rates(const xod_network *net, int64_t ncol, int64_t col0, int6
   {
     Timed tm(net, KID_RATES, s);
     k_rates<MODE><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, J, n, kf, kr, rw, (int)ncg, ntasks);
+  }
+  XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+// reaction splits per column tile of k_fused: enough work items to occupy every SM
+int fused_split(const xod_network *net, int64_t ncol) {
+  const int64_t ntiles = (ncol + kFW - 1) / kFW;
+  int64_t sp = net->force_split > 0 ? net->force_split : (ntiles >= net->sm_count ? 1 : net->sm_count / std::max<int64_t>(ntiles, 1));
+  return (int)std::max<int64_t>(1, std::min<int64_t>(sp, net->h.f.nchunk));
+}
+
+xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T, const double *P,
+                        const double *J, const double *n, double *dndt, void *workspace, cudaStream_t s) {
+  const HostTables &h = net->h;
+  FusedArgs a{};
+  a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.J = J, a.n = n;
+  a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
+  a.nsplit = fused_split(net, ncol);
+  a.log2_kb = kLog2Kb;
+  a.ldp = round_up(ncol, 32);
+  double *part = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
+  a.out = a.nsplit == 1 ? dndt : part;
+  const int64_t items = (int64_t)a.ntiles * a.nsplit;
+  const unsigned grid = (unsigned)std::min<int64_t>(items, net->sm_count);
+  const size_t smem = fused_smem_bytes(h.ns, h.f.n_acc, h.f.chunk);
+  {
+    Timed tm(net, KID_FUSED, s);
+    k_fused<<<grid, kFWarps * 32, smem, s>>>(net->fd, h.ns, a);
+  }
+  XOD_CUDA(cudaGetLastError());
+  if (a.nsplit > 1) {
+    dim3 g((unsigned)((ncol + 127) / 128), (unsigned)h.ns);
+    Timed tm(net, KID_FUSED_COMBINE, s);
+    k_fused_combine<<<g, 128, 0, s>>>(h.ns, ncol, ld, a.ldp, a.nsplit, part, dndt);
   }
   XOD_CUDA(cudaGetLastError());
   return XOD_OK;
@@ -385,7 +473,12 @@ xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const do
 
 size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol) {
   if (!net || ncol < 0) return 0;
-  return scratch_bytes(net, chunk_cols(net, ncol), true, true, true);
+  size_t b = scratch_bytes(net, chunk_cols(net, ncol), true, true, true);
+  if (net->h.f.enabled) {
+    const int ns_ = fused_split(net, ncol);
+    if (ns_ > 1) b = std::max(b, (size_t)ns_ * net->h.ns * (size_t)round_up(ncol, 32) * sizeof(double) + 256);
+  }
+  return b;
 }
 
 xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
@@ -402,6 +495,7 @@ xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, co
     return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_fused_workspace_bytes");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const bool pl = prod != nullptr;
+  if (!pl && net->fd.enabled && net->use_fused) return launch_fused(net, ncol, ld, T, P, J, n, dndt, workspace, s);
   const int64_t ldw = chunk_cols(net, ncol);
   ChunkScratch w = carve(net, workspace, ldw, true, true, pl);
   for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {

@@ -55,6 +55,53 @@ struct DevTables {
   int64_t nnz_jac;
 };
 
+// ---- tables of the single-kernel fused source path (k_fused, kernels.cuh) -------------------
+// Padded packed order: the type-sorted order with each code segment (UNI+BI | FALLOFF | PHOTO)
+// padded to a multiple of kFRxnPerWarp and the total to a multiple of the chunk size; padding
+// slots are dummy reactions without stoichiometry entries.
+constexpr int kFW = 16;           // columns per tile (one 128-byte shared-memory row)
+constexpr int kFWarps = 16;       // warps per CTA
+constexpr int kFRxnPerWarp = 4;   // reactions a warp evaluates per pass (8 lanes x 2 columns each)
+constexpr int kFPass = kFWarps * kFRxnPerWarp;  // reactions per CTA pass
+constexpr int kFSegMax = 8;       // longest row task of the production/loss phase
+constexpr int kFMaxIntervals = 32;  // distinct thermo temperature intervals the fused path supports
+
+struct FusedTask {   // one warp task of the production/loss phase: 4 row tasks run side by side
+  int32_t entry_base;  // first entry; entries are interleaved [step][4]
+  int32_t nsteps;
+  int32_t rows01;      // accumulator rows of lane groups 0, 1 (low, high 16 bits); 0xffff = idle
+  int32_t rows23;
+};
+
+struct FusedDev {
+  int32_t enabled;            // 0: fall back to the multi-kernel path
+  int32_t npad, arr_end, fo_end, ph_end;   // padded packed ranges
+  int32_t chunk, nchunk;      // reactions per chunk (multiple of kFPass), number of chunks
+  int32_t n_acc;              // accumulator rows: ns species rows + extra rows of hub species
+  int32_t n_bp;               // thermo breakpoints (distinct t_mid), n_bp + 1 intervals
+  int32_t n_extra;
+  const double *bp;           // [n_bp] ascending
+  const double *c;            // [3][npad] log2-domain forward (k_inf) coefficients
+  const double *l;            // [5][fo_end - arr_end] falloff: l0 l1 l2 fcl cN
+  const double *rev;          // [n_bp+1][7][npad] reverse-coefficient polynomial per interval
+  const int32_t *sp;          // [npad][8] r0 r1 r2 p0 p1 p2 (absent -> ns = the ones row), J row, flags
+  const int32_t *task_ptr;    // [nchunk*kFWarps + 1]
+  const FusedTask *task;
+  const uint32_t *entry;      // low 16 bits: reaction index in the chunk (chunk = zero row), high
+                              // 16 bits: top half of the high word of the double nu
+  const int32_t *extra;       // [n_extra][2] (extra accumulator row, species), grouped by species
+};
+
+struct FusedHost {
+  bool enabled = false;
+  int32_t npad = 0, arr_end = 0, fo_end = 0, ph_end = 0, chunk = 0, nchunk = 0, n_acc = 0, n_bp = 0;
+  std::vector<int32_t> pp_to_packed;   // [npad], -1 for padding
+  std::vector<double> bp, c, l, rev;
+  std::vector<int32_t> sp, task_ptr, extra;
+  std::vector<FusedTask> task;
+  std::vector<uint32_t> entry;
+};
+
 struct HostTables {
   int32_t ns = 0, ne = 0, nr = 0, n_photo = 0;
   int32_t uni_begin = 0, bi_begin = 0, fo_begin = 0, ph_begin = 0;
@@ -73,17 +120,22 @@ struct HostTables {
   std::vector<SrcSeg> src_seg;
   std::vector<int64_t> jac_term_ptr;
   std::vector<JacTerm> jac_terms;
+  FusedHost f;
 };
 
 // pack.cpp
 xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &err);
+// pack_fused.cpp: tables of the fused path for a given chunk size (0 = does not fit: disabled)
+void pack_fused(const xod_network_desc *d, HostTables &h, int chunk);
+// shared-memory bytes k_fused needs for these tables
+size_t fused_smem_bytes(int ns, int n_acc, int chunk);
 
 }  // namespace xod
 
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused
@@ -95,6 +147,10 @@ struct TimingState {
 struct xod_network {
   xod::HostTables h;
   xod::DevTables d{};
+  xod::FusedDev fd{};
+  int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
+  int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
+  int sm_count = 148;
   int device = -1;
   std::vector<void *> dev_allocs;
   int64_t chunk_cols = 0;  // 0 = default
