@@ -151,7 +151,7 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
   try {
     for (int chunk : {256, 192, 128, 64}) {
       pack_fused(desc, net->h, chunk);
-      if (net->h.f.enabled && fused_smem_bytes(net->h.ns, net->h.f.n_acc, chunk) <= kFusedSmemMax) break;
+      if (net->h.f.enabled && fused_smem_bytes(net->h.ns, net->h.f.n_acc, chunk, net->h.f.meta_cap) <= kFusedSmemMax) break;
       net->h.f.enabled = false;
     }
   } catch (const std::bad_alloc &) {
@@ -187,9 +187,15 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       fd.npad = f.npad, fd.arr_end = f.arr_end, fd.fo_end = f.fo_end, fd.ph_end = f.ph_end;
       fd.chunk = f.chunk, fd.nchunk = f.nchunk, fd.n_acc = f.n_acc, fd.n_bp = f.n_bp;
       fd.n_extra = (int32_t)(f.extra.size() / 2);
+      fd.meta_cap = f.meta_cap;
+      fd.blk_stride = f.blk_stride, fd.blk_fo_off = f.blk_fo_off, fd.blk_ph_off = f.blk_ph_off;
 #define UPF(vec, field) if (st == XOD_OK) st = upload(net, f.vec, &fd.field)
-      UPF(bp, bp); UPF(c, c); UPF(l, l); UPF(rev, rev); UPF(sp, sp); UPF(task_ptr, task_ptr);
-      UPF(task, task); UPF(entry, entry); UPF(extra, extra);
+      UPF(bp, bp); UPF(blk, blk); UPF(meta_ptr, meta_ptr); UPF(extra, extra);
+      if (st == XOD_OK) {
+        const int32_t *m = nullptr;
+        st = upload(net, f.meta, &m);
+        fd.meta = reinterpret_cast<const int4 *>(m);
+      }
 #undef UPF
       if (st == XOD_OK) {
         // the attribute is per function, not per network: always opt into the device maximum
@@ -268,9 +274,9 @@ xod_status xod_network_fused_info(const xod_network *net, int64_t *info) {
   if (!net || !info) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
   const FusedHost &f = net->h.f;
   info[0] = f.enabled, info[1] = f.chunk, info[2] = f.nchunk, info[3] = f.n_acc, info[4] = f.n_bp;
-  info[5] = f.enabled ? (int64_t)fused_smem_bytes(net->h.ns, f.n_acc, f.chunk) : 0;
-  info[6] = f.npad, info[7] = (int64_t)f.task.size(), info[8] = (int64_t)f.entry.size();
-  info[9] = (int64_t)(f.rev.size() * sizeof(double));
+  info[5] = f.enabled ? (int64_t)fused_smem_bytes(net->h.ns, f.n_acc, f.chunk, f.meta_cap) : 0;
+  info[6] = f.npad, info[7] = f.n_tasks, info[8] = f.n_entries;
+  info[9] = (int64_t)f.blk.size();
   return XOD_OK;
 }
 
@@ -378,7 +384,7 @@ xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const 
   a.out = a.nsplit == 1 ? dndt : part;
   const int64_t items = (int64_t)a.ntiles * a.nsplit;
   const unsigned grid = (unsigned)std::min<int64_t>(items, net->sm_count);
-  const size_t smem = fused_smem_bytes(h.ns, h.f.n_acc, h.f.chunk);
+  const size_t smem = fused_smem_bytes(h.ns, h.f.n_acc, h.f.chunk, h.f.meta_cap);
   {
     Timed tm(net, KID_FUSED, s);
     k_fused<<<grid, kFWarps * 32, smem, s>>>(net->fd, h.ns, a);

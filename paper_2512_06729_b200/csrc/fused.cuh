@@ -6,11 +6,13 @@
 //   n_s   [ns + 1]      number densities of the tile (+ a row of ones for absent species slots)
 //   acc_s [n_acc]       dn/dt accumulators (+ extra rows of hub species, see pack_fused.cpp)
 //   q_s   [2][chunk+1]  net rates of progress of the current / next chunk (+ a zero row)
+//   meta_s[2][meta_cap] the production/loss schedule of the current / next chunk (cp.async)
 // Per chunk: phase A (FP64-pipe bound) evaluates k_f, k_r and q = k_f prod n - k_r prod n for
 // chunk x 16 (reaction, column) pairs, 8 lanes x 2 columns per reaction, 4 reactions per warp
-// pass, reaction parameters read once per 64 pairs; one __syncthreads; phase B (shared-memory
-// bound) runs the packer's row tasks: lane groups sum nu q over <= kFSegMax entries and add the
-// result to "their" accumulator row.  q is double-buffered, so warps that finish phase B early
+// pass; the parameters of those 4 reactions are one contiguous block read with 16-byte loads at
+// immediate offsets.  One __syncthreads; phase B (shared-memory bound) runs the packer's row
+// tasks: lane groups sum nu q over <= kFSegMax entries and add the result to "their"
+// accumulator row.  q and the schedule are double-buffered, so warps that finish phase B early
 // start phase A of the next chunk at once.  No atomics; the summation order is fixed.
 //
 //   UNI/BI   log2 k_f = c0 + c1 log2 T + c2 / T                                  (Eq. 7)
@@ -37,20 +39,18 @@ struct FusedArgs {
 };
 
 __device__ __forceinline__ double2 lds2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
-
-// seven reverse coefficients of reaction pp in interval g
-struct Rev7 { double c[7]; };
-__device__ __forceinline__ Rev7 load_rev(const FusedDev &f, int g, int pp) {
-  Rev7 r;
-  const double *base = f.rev + ((size_t)g * 7) * f.npad + pp;
-#pragma unroll
-  for (int k = 0; k < 7; ++k) r.c[k] = __ldg(base + (size_t)k * f.npad);
-  return r;
+__device__ __forceinline__ double2 ldg2(const unsigned char *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
 }
-// z-polynomial: C0 + C1 log2 T + C2 / T - T (D2 + T (D3 + T (D4 + T D5)))
-__device__ __forceinline__ double rev_eval(const Rev7 &r, double T, double l2T, double invT) {
-  const double poly = fma(T, fma(T, fma(T, r.c[6], r.c[5]), r.c[4]), r.c[3]);
-  return fma(r.c[2], invT, fma(r.c[1], l2T, fma(-T, poly, r.c[0])));
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+
+// log2 k_r (UNI/BI) or z (FALLOFF) from the block of interval g
+__device__ __forceinline__ double rev_eval(const unsigned char *blk, int slot16, double c0r /*C0*/, double T,
+                                           double l2T, double invT) {
+  const double2 c12 = ldg2(blk + 4 * 64 + slot16), d23 = ldg2(blk + 5 * 64 + slot16), d45 = ldg2(blk + 6 * 64 + slot16);
+  const double poly = fma(T, fma(T, fma(T, d45.y, d45.x), d23.y), d23.x);
+  return fma(c12.y, invT, fma(c12.x, l2T, fma(-T, poly, c0r)));
 }
 
 __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, FusedArgs a) {
@@ -58,12 +58,14 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
   double *n_s = reinterpret_cast<double *>(smem_raw);
   double *acc_s = n_s + (size_t)(ns + 1) * kFW;
   double *q_s = acc_s + (size_t)f.n_acc * kFW;
-  double *cT = q_s + (size_t)2 * (f.chunk + 1) * kFW;
+  int4 *meta_s = reinterpret_cast<int4 *>(q_s + (size_t)2 * (f.chunk + 1) * kFW);
+  double *cT = reinterpret_cast<double *>(meta_s + 2 * f.meta_cap);
   double *cL2T = cT + kFW, *cInvT = cL2T + kFW, *cLM = cInvT + kFW;
   int *cG = reinterpret_cast<int *>(cLM + kFW);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int grp = lane >> 3, l2 = (lane & 7) * 2;  // lane group (reaction slot) and first column
+  const int slot16 = grp * 16;
   const int qrows = f.chunk + 1;
 
   for (int item = blockIdx.x; item < a.ntiles * a.nsplit; item += gridDim.x) {
@@ -99,77 +101,104 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
     __syncthreads();
     const double T0 = cT[l2], T1 = cT[l2 + 1], lT0 = cL2T[l2], lT1 = cL2T[l2 + 1];
     const double iT0 = cInvT[l2], iT1 = cInvT[l2 + 1];
-    const int g0 = cG[l2], g1 = cG[l2 + 1];
     const int64_t gc0 = min(col0 + l2, a.ncol - 1), gc1 = min(col0 + l2 + 1, a.ncol - 1);
+    const unsigned char *blk0 = f.blk + (size_t)cG[l2] * f.blk_stride;
+    const unsigned char *blk1 = f.blk + (size_t)cG[l2 + 1] * f.blk_stride;
+    const bool same_g = blk0 == blk1;
+    const double *n_l = n_s + l2;
 
     for (int k = k_begin; k < k_end; ++k) {
-      double *qb = q_s + (size_t)((k - k_begin) & 1) * qrows * kFW;
+      const int buf = (k - k_begin) & 1;
+      double *qb = q_s + (size_t)buf * qrows * kFW;
+      int4 *mb = meta_s + (size_t)buf * f.meta_cap;
+      // schedule of this chunk -> shared memory, overlapped with phase A
+      {
+        const int m0 = __ldg(f.meta_ptr + k), m1 = __ldg(f.meta_ptr + k + 1);
+        for (int u = m0 + tid; u < m1; u += kFWarps * 32) cp_async16(mb + (u - m0), f.meta + u);
+      }
       // ------------------------------------------------------------ phase A
       const int pp_chunk = k * f.chunk;
+#pragma unroll 1
       for (int pass = 0; pass < f.chunk / kFPass; ++pass) {
-        const int rloc = pass * kFPass + warp * kFRxnPerWarp + grp;
-        const int pp = pp_chunk + rloc;
-        const int ppw = pp_chunk + pass * kFPass + warp * kFRxnPerWarp;  // warp-uniform
-        if (ppw >= f.ph_end) break;                                    // only padding left
-        const int4 sa = __ldg(reinterpret_cast<const int4 *>(f.sp + (size_t)pp * 8));
-        const int4 sb = __ldg(reinterpret_cast<const int4 *>(f.sp + (size_t)pp * 8 + 4));
+        const int rbase = pass * kFPass + warp * kFRxnPerWarp;
+        const int ppw = pp_chunk + rbase;  // first of the warp's 4 reactions (one segment)
+        if (ppw >= f.ph_end) break;        // only padding left
         double kf0, kf1, kr0, kr1;
+        int4 sa, sb;
         if (ppw < f.fo_end) {
-          const double c0 = __ldg(f.c + pp), c1 = __ldg(f.c + f.npad + pp), c2 = __ldg(f.c + 2 * (size_t)f.npad + pp);
-          const double y0 = fma(c2, iT0, fma(c1, lT0, c0)), y1 = fma(c2, iT1, fma(c1, lT1, c0));
-          const Rev7 ra = load_rev(f, g0, pp);
-          double z0 = rev_eval(ra, T0, lT0, iT0), z1;
-          if (g1 == g0) {
-            z1 = rev_eval(ra, T1, lT1, iT1);
+          const bool arr = ppw < f.arr_end;
+          const size_t off = arr ? (size_t)(ppw >> 2) * kFBlkArr
+                                 : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
+          const unsigned char *b0 = blk0 + off;
+          sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
+          sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64 + slot16));
+          const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
+          const double y0 = fma(c2C.x, iT0, fma(c01.y, lT0, c01.x)), y1 = fma(c2C.x, iT1, fma(c01.y, lT1, c01.x));
+          const double z0 = rev_eval(b0, slot16, c2C.y, T0, lT0, iT0);
+          double z1;
+          if (same_g) {
+            z1 = rev_eval(b0, slot16, c2C.y, T1, lT1, iT1);
           } else {
-            const Rev7 rb = load_rev(f, g1, pp);
-            z1 = rev_eval(rb, T1, lT1, iT1);
+            const unsigned char *b1 = blk1 + off;
+            z1 = rev_eval(b1, slot16, ldg2(b1 + 3 * 64 + slot16).y, T1, lT1, iT1);
           }
-          if (ppw < f.arr_end) {  // UNI, BI
-            kf0 = xexp2(y0), kf1 = xexp2(y1);
-            kr0 = xexp2(z0), kr1 = xexp2(z1);
-          } else {                // FALLOFF
-            const int q = pp - f.arr_end, nfo = f.fo_end - f.arr_end;
-            const double m0 = __ldg(f.l + q), m1 = __ldg(f.l + nfo + q), m2 = __ldg(f.l + 2 * nfo + q);
-            const double fcl = __ldg(f.l + 3 * nfo + q), cN = __ldg(f.l + 4 * nfo + q);
-            const double w0 = fma(m2, iT0, fma(m1, lT0, m0)) + cLM[l2];
-            const double w1 = fma(m2, iT1, fma(m1, lT1, m0)) + cLM[l2 + 1];
+          if (arr) {  // UNI, BI
+            const unsigned m = max(max(xexp2_mag(y0), xexp2_mag(y1)), max(xexp2_mag(z0), xexp2_mag(z1)));
+            if (m < kExp2FastMax) {
+              kf0 = xexp2_fast(y0), kf1 = xexp2_fast(y1), kr0 = xexp2_fast(z0), kr1 = xexp2_fast(z1);
+            } else {
+              kf0 = xexp2_slow(y0), kf1 = xexp2_slow(y1), kr0 = xexp2_slow(z0), kr1 = xexp2_slow(z1);
+            }
+          } else {    // FALLOFF
+            const double2 m01 = ldg2(b0 + 7 * 64 + slot16), m2f = ldg2(b0 + 8 * 64 + slot16);
+            const double cN = ldg2(b0 + 9 * 64 + slot16).x;
+            const double w0 = fma(m2f.x, iT0, fma(m01.y, lT0, m01.x)) + cLM[l2];
+            const double w1 = fma(m2f.x, iT1, fma(m01.y, lT1, m01.x)) + cLM[l2 + 1];
             const double lp0 = w0 - y0, lp1 = w1 - y1;             // log2 Pr
             const double x0 = lp0 * cN, x1 = lp1 * cN;
-            const double lF0 = fcl / fma(x0, x0, 1.0), lF1 = fcl / fma(x1, x1, 1.0);
+            const double lF0 = m2f.y / fma(x0, x0, 1.0), lF1 = m2f.y / fma(x1, x1, 1.0);
             const double d0 = 1.0 / (1.0 + xexp2(-fabs(lp0))), d1 = 1.0 / (1.0 + xexp2(-fabs(lp1)));
             const double ym0 = fmin(w0, y0) + lF0, ym1 = fmin(w1, y1) + lF1;
             kf0 = xexp2(ym0) * d0, kf1 = xexp2(ym1) * d1;
             kr0 = xexp2(ym0 + z0) * d0, kr1 = xexp2(ym1 + z1) * d1;
           }
         } else {                  // PHOTO
+          const unsigned char *b0 = f.blk + (size_t)f.blk_ph_off + (size_t)((ppw - f.fo_end) >> 2) * kFBlkPh;
+          sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
+          sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64 + slot16));
           kf0 = a.J[(size_t)sb.z * a.ld + gc0], kf1 = a.J[(size_t)sb.z * a.ld + gc1];
           kr0 = kr1 = 0.0;
         }
-        double2 v = lds2(n_s + sa.x * kFW + l2);
+        // a7: rates of progress (absent slots read the row of ones)
+        double2 v = lds2(n_l + sa.x * kFW);
         double qf0 = kf0 * v.x, qf1 = kf1 * v.y;
-        if (sa.y != ns) { v = lds2(n_s + sa.y * kFW + l2); qf0 *= v.x, qf1 *= v.y; }
-        if (sa.z != ns) { v = lds2(n_s + sa.z * kFW + l2); qf0 *= v.x, qf1 *= v.y; }
-        v = lds2(n_s + sa.w * kFW + l2);
+        if (sa.y != ns) { v = lds2(n_l + sa.y * kFW); qf0 *= v.x, qf1 *= v.y; }
+        if (sa.z != ns) { v = lds2(n_l + sa.z * kFW); qf0 *= v.x, qf1 *= v.y; }
+        v = lds2(n_l + sa.w * kFW);
         double qr0 = kr0 * v.x, qr1 = kr1 * v.y;
-        if (sb.x != ns) { v = lds2(n_s + sb.x * kFW + l2); qr0 *= v.x, qr1 *= v.y; }
-        if (sb.y != ns) { v = lds2(n_s + sb.y * kFW + l2); qr0 *= v.x, qr1 *= v.y; }
-        *reinterpret_cast<double2 *>(qb + (size_t)rloc * kFW + l2) = make_double2(qf0 - qr0, qf1 - qr1);
+        if (sb.x != ns) { v = lds2(n_l + sb.x * kFW); qr0 *= v.x, qr1 *= v.y; }
+        if (sb.y != ns) { v = lds2(n_l + sb.y * kFW); qr0 *= v.x, qr1 *= v.y; }
+        *reinterpret_cast<double2 *>(qb + (size_t)(rbase + grp) * kFW + l2) = make_double2(qf0 - qr0, qf1 - qr1);
       }
+      cp_async_wait_all();
       __syncthreads();
       // ------------------------------------------------------------ phase B
-      const int t_begin = __ldg(f.task_ptr + (size_t)k * kFWarps + warp);
-      const int t_end = __ldg(f.task_ptr + (size_t)k * kFWarps + warp + 1);
+      const int *hdr = reinterpret_cast<const int *>(mb);
+      const int t_begin = hdr[warp], t_end = hdr[warp + 1];
+      const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + hdr[kFWarps + 1]) + grp;
+      const double *q_l = qb + l2;
+#pragma unroll 1
       for (int t = t_begin; t < t_end; ++t) {
-        const int4 tk = __ldg(reinterpret_cast<const int4 *>(f.task + t));
+        const int4 tk = mb[kFMetaHdr / 4 + t];
         const unsigned rows = (grp & 2) ? (unsigned)tk.w : (unsigned)tk.z;
         const int row = (int)((grp & 1) ? rows >> 16 : rows & 0xffffu);
-        const uint32_t *e = f.entry + tk.x + grp;
+        const unsigned *e = ent + tk.x;
         double s0 = 0.0, s1 = 0.0;
+#pragma unroll 1
         for (int st = 0; st < tk.y; ++st) {
-          const uint32_t en = __ldg(e + st * 4);
+          const unsigned en = e[st * 4];
           const double nu = __hiloint2double((int)(en & 0xffff0000u), 0);
-          const double2 qv = lds2(qb + (size_t)(en & 0xffffu) * kFW + l2);
+          const double2 qv = lds2(q_l + (en & 0xffffu) * kFW);
           s0 = fma(nu, qv.x, s0), s1 = fma(nu, qv.y, s1);
         }
         if (row != 0xffff) {

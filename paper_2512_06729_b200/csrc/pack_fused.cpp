@@ -39,10 +39,11 @@ void scaled_nasa(const double *a, long double b[7]) {
 }
 }  // namespace
 
-size_t fused_smem_bytes(int ns, int n_acc, int chunk) {
-  // n tile (+ ones row) | accumulator rows | two q buffers (+ zero row each) | column scalars
+size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap) {
+  // n tile (+ ones row) | accumulator rows | two q buffers (+ zero row each) | two chunk schedules
+  // | column scalars
   return ((size_t)(ns + 1) + (size_t)n_acc + 2 * (size_t)(chunk + 1)) * kFW * sizeof(double) +
-         (size_t)kFW * (4 * sizeof(double) + sizeof(int32_t));
+         2 * (size_t)meta_cap * 16 + (size_t)kFW * (4 * sizeof(double) + sizeof(int32_t));
 }
 
 void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
@@ -79,63 +80,63 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
   for (int pp = 0; pp < f.npad; ++pp)
     if (f.pp_to_packed[pp] >= 0) packed_to_pp[f.pp_to_packed[pp]] = pp;
 
-  // ---- forward coefficients, falloff extras, species slots
-  const size_t np = (size_t)f.npad, nfo_pad = (size_t)(f.fo_end - f.arr_end);
-  f.c.assign(3 * np, 0.0);
-  f.l.assign(5 * std::max<size_t>(nfo_pad, 1), 0.0);
-  f.sp.assign(8 * np, ns);  // absent species -> the ones row of the n tile
-  for (int pp = 0; pp < f.npad; ++pp) {
-    int32_t *s = &f.sp[(size_t)pp * 8];
-    s[6] = 0, s[7] = 0;  // padding slots of the PHOTO segment read row 0 of J (result unused)
-    const int p = f.pp_to_packed[pp];
-    if (p < 0) continue;
-    for (int a = 0; a < 6; ++a)
-      if (h.sp[(size_t)p * 6 + a] >= 0) s[a] = h.sp[(size_t)p * 6 + a];
-    s[7] = h.flags[p];
-    f.c[pp] = h.c0[p], f.c[np + pp] = h.c1[p], f.c[2 * np + pp] = h.c2[p];
-    if (p >= h.ph_begin) s[6] = h.photo_row[p - h.ph_begin];
-    if (p >= h.fo_begin && p < h.ph_begin) {
-      const size_t q = (size_t)(pp - f.arr_end);
-      const int fo = p - h.fo_begin;
-      f.l[q] = h.l0[fo], f.l[nfo_pad + q] = h.l1[fo], f.l[2 * nfo_pad + q] = h.l2[fo];
-      f.l[3 * nfo_pad + q] = h.fcl[fo], f.l[4 * nfo_pad + q] = h.cN[fo];
-    }
-  }
-
-  // ---- reverse-coefficient table [interval][7][npad]
+  // ---- parameter blocks [interval][group], see xod_internal.h
+  //   reverse coefficients, per interval (seven numbers per reaction):
   //   UNI/BI : C0 = c0 + dB0, C1 = c1 - dB1, C2 = c2 + dB6   (k_f folded in: one exp2 gives k_r)
   //   FALLOFF: C0 = dB0, C1 = -dB1, C2 = dB6                 (pure z; added to log2 k_f in the kernel)
-  //   irreversible, photolysis, padding: C0 = -inf, rest 0   (k_r = 0)
+  //   irreversible, padding: C0 = -inf, rest 0               (k_r = 0)
   const int ng = f.n_bp + 1;
-  f.rev.assign((size_t)ng * 7 * np, 0.0);
+  const int64_t n_arr_g = f.arr_end / kFRxnPerWarp, n_fo_g = (f.fo_end - f.arr_end) / kFRxnPerWarp,
+                n_ph_g = (f.ph_end - f.fo_end) / kFRxnPerWarp;
+  f.blk_fo_off = n_arr_g * kFBlkArr;
+  f.blk_ph_off = f.blk_fo_off + n_fo_g * kFBlkFo;
+  f.blk_stride = f.blk_ph_off + n_ph_g * kFBlkPh;
+  f.blk.assign((size_t)ng * f.blk_stride, 0);
   std::vector<long double> blo((size_t)ns * 7), bhi((size_t)ns * 7);
   for (int i = 0; i < ns; ++i) {
     scaled_nasa(d->nasa_lo + (size_t)7 * i, &blo[(size_t)i * 7]);
     scaled_nasa(d->nasa_hi + (size_t)7 * i, &bhi[(size_t)i * 7]);
   }
   for (int g = 0; g < ng; ++g)
-    for (int pp = 0; pp < f.npad; ++pp) {
-      double *out = &f.rev[((size_t)g * 7) * np + pp];
+    for (int pp = 0; pp < f.ph_end; ++pp) {
+      const int seg = pp < f.arr_end ? 0 : pp < f.fo_end ? 1 : 2;
+      const int first = seg == 0 ? 0 : seg == 1 ? f.arr_end : f.fo_end;
+      const int64_t off = seg == 0 ? 0 : seg == 1 ? f.blk_fo_off : f.blk_ph_off;
+      const int bsz = seg == 0 ? kFBlkArr : seg == 1 ? kFBlkFo : kFBlkPh;
+      unsigned char *blk = &f.blk[(size_t)g * f.blk_stride + off + (size_t)((pp - first) / kFRxnPerWarp) * bsz];
+      const int slot = (pp - first) % kFRxnPerWarp;
       const int p = f.pp_to_packed[pp];
-      if (p < 0 || p >= h.ph_begin || !(h.flags[p] & 1)) {
-        out[0] = -INFINITY;
-        continue;
+      int32_t sp8[8] = {ns, ns, ns, ns, ns, ns, 0, 0};  // absent species -> the ones row of the n tile
+      double v[16] = {0, 0, 0, -INFINITY, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      if (p >= 0) {
+        for (int a = 0; a < 6; ++a)
+          if (h.sp[(size_t)p * 6 + a] >= 0) sp8[a] = h.sp[(size_t)p * 6 + a];
+        sp8[7] = h.flags[p];
+        if (p >= h.ph_begin) sp8[6] = h.photo_row[p - h.ph_begin];
+        v[0] = h.c0[p], v[1] = h.c1[p], v[2] = h.c2[p];
+        if (p < h.ph_begin && (h.flags[p] & 1)) {
+          long double db[7] = {0, 0, 0, 0, 0, 0, 0};
+          for (int a = 0; a < 6; ++a) {
+            const int i = h.sp[(size_t)p * 6 + a];
+            if (i < 0) continue;
+            const long double *b = (g <= bp_of[i] ? &blo[(size_t)i * 7] : &bhi[(size_t)i * 7]);
+            for (int k = 0; k < 7; ++k) db[k] += a < 3 ? -b[k] : b[k];
+          }
+          const bool fold = p < h.fo_begin;
+          v[3] = (double)((fold ? (long double)h.c0[p] : 0.0L) + db[0]);
+          v[4] = (double)((fold ? (long double)h.c1[p] : 0.0L) - db[1]);
+          v[5] = (double)((fold ? (long double)h.c2[p] : 0.0L) + db[6]);
+          v[6] = (double)db[2], v[7] = (double)db[3], v[8] = (double)db[4], v[9] = (double)db[5];
+        }
+        if (seg == 1) {
+          const int fo = p - h.fo_begin;
+          v[10] = h.l0[fo], v[11] = h.l1[fo], v[12] = h.l2[fo], v[13] = h.fcl[fo], v[14] = h.cN[fo];
+        }
       }
-      long double db[7] = {0, 0, 0, 0, 0, 0, 0};
-      for (int a = 0; a < 6; ++a) {
-        const int i = h.sp[(size_t)p * 6 + a];
-        if (i < 0) continue;
-        const long double *b = (g <= bp_of[i] ? &blo[(size_t)i * 7] : &bhi[(size_t)i * 7]);
-        for (int k = 0; k < 7; ++k) db[k] += a < 3 ? -b[k] : b[k];
-      }
-      const bool fold = p < h.fo_begin;
-      out[0] = (double)((fold ? (long double)h.c0[p] : 0.0L) + db[0]);
-      out[1 * np] = (double)((fold ? (long double)h.c1[p] : 0.0L) - db[1]);
-      out[2 * np] = (double)((fold ? (long double)h.c2[p] : 0.0L) + db[6]);
-      out[3 * np] = (double)db[2];
-      out[4 * np] = (double)db[3];
-      out[5 * np] = (double)db[4];
-      out[6 * np] = (double)db[5];
+      std::memcpy(blk + 0 * 64 + slot * 16, sp8, 16);
+      std::memcpy(blk + 1 * 64 + slot * 16, sp8 + 4, 16);
+      const int npair = seg == 0 ? 5 : seg == 1 ? 8 : 0;
+      for (int u = 0; u < npair; ++u) std::memcpy(blk + (2 + u) * 64 + slot * 16, v + 2 * u, 16);
     }
 
   // ---- production/loss schedule
@@ -181,9 +182,9 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
 
   struct Seg { int32_t row; const uint32_t *ent; int len; };
   const uint32_t zero_entry = (uint32_t)chunk;  // nu bits 0 (= +0.0), the zero row of q
-  f.task_ptr.assign((size_t)nchunk * kFWarps + 1, 0);
-  f.task.clear();
-  f.entry.clear();
+  f.meta_ptr.assign((size_t)nchunk + 1, 0);
+  f.meta.clear();
+  f.meta_cap = 0, f.n_tasks = 0, f.n_entries = 0;
   for (int k = 0; k < nchunk; ++k) {
     std::vector<Seg> segs;
     for (const Row &r : rows[k]) {
@@ -197,10 +198,11 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
     // warp tasks of 4 similar-length segments, dealt to the least-loaded warp (longest first)
     std::vector<std::vector<FusedTask>> per_warp(kFWarps);
     std::vector<int> load(kFWarps, 0);
+    std::vector<uint32_t> entries;
     for (size_t s0 = 0; s0 < segs.size(); s0 += 4) {
       const int cnt = (int)std::min<size_t>(4, segs.size() - s0), nsteps = segs[s0].len;
       FusedTask t;
-      t.entry_base = (int32_t)f.entry.size();
+      t.entry_off = (int32_t)entries.size();
       t.nsteps = nsteps;
       uint32_t r[4] = {0xffffu, 0xffffu, 0xffffu, 0xffffu};
       for (int g = 0; g < cnt; ++g) r[g] = (uint32_t)segs[s0 + g].row;
@@ -208,15 +210,29 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
       t.rows23 = (int32_t)(r[2] | (r[3] << 16));
       for (int st = 0; st < nsteps; ++st)
         for (int g = 0; g < 4; ++g)
-          f.entry.push_back(g < cnt && st < segs[s0 + g].len ? segs[s0 + g].ent[st] : zero_entry);
+          entries.push_back(g < cnt && st < segs[s0 + g].len ? segs[s0 + g].ent[st] : zero_entry);
       const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
       load[w] += nsteps + 2;
       per_warp[w].push_back(t);
     }
+    // blob: header (17 task offsets per warp, task count) | tasks | entries, 16-byte units
+    std::vector<int32_t> blob(kFMetaHdr, 0);
+    int nt = 0;
     for (int w = 0; w < kFWarps; ++w) {
-      f.task.insert(f.task.end(), per_warp[w].begin(), per_warp[w].end());
-      f.task_ptr[(size_t)k * kFWarps + w + 1] = (int32_t)f.task.size();
+      blob[w] = nt;
+      nt += (int)per_warp[w].size();
     }
+    blob[kFWarps] = nt, blob[kFWarps + 1] = nt;
+    for (int w = 0; w < kFWarps; ++w)
+      for (const FusedTask &t : per_warp[w]) {
+        blob.push_back(t.entry_off), blob.push_back(t.nsteps), blob.push_back(t.rows01), blob.push_back(t.rows23);
+      }
+    for (uint32_t e : entries) blob.push_back((int32_t)e);
+    while (blob.size() % 4) blob.push_back((int32_t)zero_entry);
+    f.meta.insert(f.meta.end(), blob.begin(), blob.end());
+    f.meta_ptr[k + 1] = (int32_t)(f.meta.size() / 4);
+    f.meta_cap = std::max<int32_t>(f.meta_cap, (int32_t)(blob.size() / 4));
+    f.n_tasks += nt, f.n_entries += (int64_t)entries.size();
   }
   f.enabled = true;
 }

@@ -2,6 +2,7 @@
 // Part of libxodiac (the CUDA product path).  Shares nothing with oracle/.
 #pragma once
 #include <cstdint>
+#include <vector_types.h>
 #include <string>
 #include <vector>
 
@@ -63,15 +64,24 @@ constexpr int kFW = 16;           // columns per tile (one 128-byte shared-memor
 constexpr int kFWarps = 16;       // warps per CTA
 constexpr int kFRxnPerWarp = 4;   // reactions a warp evaluates per pass (8 lanes x 2 columns each)
 constexpr int kFPass = kFWarps * kFRxnPerWarp;  // reactions per CTA pass
-constexpr int kFSegMax = 8;       // longest row task of the production/loss phase
+constexpr int kFSegMax = 16;      // longest row task of the production/loss phase
 constexpr int kFMaxIntervals = 32;  // distinct thermo temperature intervals the fused path supports
 
 struct FusedTask {   // one warp task of the production/loss phase: 4 row tasks run side by side
-  int32_t entry_base;  // first entry; entries are interleaved [step][4]
+  int32_t entry_off;   // first entry (in words from the start of the chunk's entry section);
+                       // entries are interleaved [step][4]
   int32_t nsteps;
   int32_t rows01;      // accumulator rows of lane groups 0, 1 (low, high 16 bits); 0xffff = idle
   int32_t rows23;
 };
+
+// Parameter blocks: one block per (thermo interval, group of kFRxnPerWarp reactions), made of
+// 16-byte units indexed [unit][reaction in group]: sa, sb (species slots as int4), then double2
+// pairs (c0,c1) (c2,C0) (C1,C2) (D2,D3) (D4,D5) and, for FALLOFF, (m0,m1) (m2,fcl) (cN,-).
+constexpr int kFBlkArr = 7 * 64;   // bytes of a UNI/BI block
+constexpr int kFBlkFo = 10 * 64;   // bytes of a FALLOFF block
+constexpr int kFBlkPh = 2 * 64;    // bytes of a PHOTO block (species slots only)
+constexpr int kFMetaHdr = 20;      // int32 words of a chunk's schedule header (17 warp offsets, task count)
 
 struct FusedDev {
   int32_t enabled;            // 0: fall back to the multi-kernel path
@@ -80,26 +90,27 @@ struct FusedDev {
   int32_t n_acc;              // accumulator rows: ns species rows + extra rows of hub species
   int32_t n_bp;               // thermo breakpoints (distinct t_mid), n_bp + 1 intervals
   int32_t n_extra;
+  int32_t meta_cap;           // 16-byte units of the largest chunk schedule
+  int64_t blk_stride;         // bytes of one interval's parameter blocks
+  int64_t blk_fo_off, blk_ph_off;  // byte offsets of the FALLOFF and PHOTO blocks in an interval
   const double *bp;           // [n_bp] ascending
-  const double *c;            // [3][npad] log2-domain forward (k_inf) coefficients
-  const double *l;            // [5][fo_end - arr_end] falloff: l0 l1 l2 fcl cN
-  const double *rev;          // [n_bp+1][7][npad] reverse-coefficient polynomial per interval
-  const int32_t *sp;          // [npad][8] r0 r1 r2 p0 p1 p2 (absent -> ns = the ones row), J row, flags
-  const int32_t *task_ptr;    // [nchunk*kFWarps + 1]
-  const FusedTask *task;
-  const uint32_t *entry;      // low 16 bits: reaction index in the chunk (chunk = zero row), high
-                              // 16 bits: top half of the high word of the double nu
+  const unsigned char *blk;   // [n_bp+1] x blk_stride
+  const int32_t *meta_ptr;    // [nchunk + 1] in 16-byte units into meta
+  const int4 *meta;           // per chunk: header | tasks | entries
   const int32_t *extra;       // [n_extra][2] (extra accumulator row, species), grouped by species
 };
 
 struct FusedHost {
   bool enabled = false;
   int32_t npad = 0, arr_end = 0, fo_end = 0, ph_end = 0, chunk = 0, nchunk = 0, n_acc = 0, n_bp = 0;
+  int32_t meta_cap = 0;
+  int64_t blk_stride = 0, blk_fo_off = 0, blk_ph_off = 0;
+  int64_t n_tasks = 0, n_entries = 0;
   std::vector<int32_t> pp_to_packed;   // [npad], -1 for padding
-  std::vector<double> bp, c, l, rev;
-  std::vector<int32_t> sp, task_ptr, extra;
-  std::vector<FusedTask> task;
-  std::vector<uint32_t> entry;
+  std::vector<double> bp;
+  std::vector<unsigned char> blk;
+  std::vector<int32_t> meta_ptr, extra;
+  std::vector<int32_t> meta;           // 4 words per 16-byte unit
 };
 
 struct HostTables {
@@ -128,7 +139,7 @@ xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &e
 // pack_fused.cpp: tables of the fused path for a given chunk size (0 = does not fit: disabled)
 void pack_fused(const xod_network_desc *d, HostTables &h, int chunk);
 // shared-memory bytes k_fused needs for these tables
-size_t fused_smem_bytes(int ns, int n_acc, int chunk);
+size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap);
 
 }  // namespace xod
 
