@@ -149,7 +149,7 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
   net->device = cuda_device;
   // tables of the single-kernel fused path: the largest chunk whose shared memory fits one CTA
   try {
-    for (int chunk : {256, 192, 128, 64}) {
+    for (int chunk : {4 * kFPass, 3 * kFPass, 2 * kFPass, kFPass}) {
       pack_fused(desc, net->h, chunk);
       if (net->h.f.enabled && fused_smem_bytes(net->h.ns, net->h.f.n_acc, chunk, net->h.f.meta_cap) <= kFusedSmemMax) break;
       net->h.f.enabled = false;
@@ -287,6 +287,10 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
     net->chunk_cols = value;
     return XOD_OK;
   }
+  if (knob == 99) {  // undocumented: ablation switches of k_fused (profiling only)
+    net->debug = value;
+    return XOD_OK;
+  }
   if (knob == XOD_TUNE_SPLIT) {
     if (value < 0) return fail(XOD_ERR_INVALID_ARG, "split must be >= 0");
     net->force_split = value;
@@ -379,6 +383,7 @@ xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const 
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
   a.nsplit = fused_split(net, ncol);
   a.log2_kb = kLog2Kb;
+  a.debug = (int32_t)net->debug;
   a.ldp = round_up(ncol, 32);
   double *part = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
   a.out = a.nsplit == 1 ? dndt : part;

@@ -35,6 +35,7 @@ struct FusedArgs {
   double *out;                // nsplit == 1: dndt [ns][ld]; else partial sums [nsplit][ns][ldp]
   int64_t ldp;                // pitch of the partial sums
   int32_t ntiles, nsplit;
+  int32_t debug;              // ablation switches for profiling (XOD_TUNE_DEBUG); 0 in production
   double log2_kb;
 };
 
@@ -42,6 +43,9 @@ __device__ __forceinline__ double2 lds2(const double *p) { return *reinterpret_c
 __device__ __forceinline__ double2 ldg2(const unsigned char *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
@@ -90,7 +94,8 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
     {
       const int c = tid & (kFW - 1);
       const int64_t gc = min(col0 + c, a.ncol - 1);
-      for (int i = tid >> 4; i < ns; i += (kFWarps * 32) >> 4) n_s[i * kFW + c] = a.n[(size_t)i * a.ld + gc];
+      // all loads of the tile in flight at once (cp.async), not one round trip per row
+      for (int i = tid >> 4; i < ns; i += (kFWarps * 32) >> 4) cp_async8(n_s + i * kFW + c, a.n + (size_t)i * a.ld + gc);
       for (int i = tid; i < f.n_acc * kFW; i += kFWarps * 32) acc_s[i] = 0.0;
       if (tid < kFW) {
         n_s[ns * kFW + tid] = 1.0;
@@ -98,6 +103,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
         q_s[(size_t)(qrows + f.chunk) * kFW + tid] = 0.0;
       }
     }
+    cp_async_wait_all();
     __syncthreads();
     const double T0 = cT[l2], T1 = cT[l2 + 1], lT0 = cL2T[l2], lT1 = cL2T[l2 + 1];
     const double iT0 = cInvT[l2], iT1 = cInvT[l2 + 1];
@@ -119,17 +125,19 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       // ------------------------------------------------------------ phase A
       const int pp_chunk = k * f.chunk;
 #pragma unroll 1
-      for (int pass = 0; pass < f.chunk / kFPass; ++pass) {
+      for (int pass_ = 0; pass_ < (f.chunk / kFPass << ((a.debug >> 5) & 1)); ++pass_) {
+        const int pass = pass_ >> ((a.debug >> 5) & 1);
         const int rbase = pass * kFPass + warp * kFRxnPerWarp;
         const int ppw = pp_chunk + rbase;  // first of the warp's 4 reactions (one segment)
         if (ppw >= f.ph_end) break;        // only padding left
+        if (a.debug & 16) continue;
         double kf0, kf1, kr0, kr1;
         int4 sa, sb;
         if (ppw < f.fo_end) {
           const bool arr = ppw < f.arr_end;
           const size_t off = arr ? (size_t)(ppw >> 2) * kFBlkArr
                                  : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
-          const unsigned char *b0 = blk0 + off;
+          const unsigned char *b0 = blk0 + ((a.debug & 8) ? (size_t)0 : off);
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
           sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64 + slot16));
           const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
@@ -144,7 +152,9 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           }
           if (arr) {  // UNI, BI
             const unsigned m = max(max(xexp2_mag(y0), xexp2_mag(y1)), max(xexp2_mag(z0), xexp2_mag(z1)));
-            if (m < kExp2FastMax) {
+            if (a.debug & 2) {
+              kf0 = y0, kf1 = y1, kr0 = z0, kr1 = z1;
+            } else if (m < kExp2FastMax) {
               kf0 = xexp2_fast(y0), kf1 = xexp2_fast(y1), kr0 = xexp2_fast(z0), kr1 = xexp2_fast(z1);
             } else {
               kf0 = xexp2_slow(y0), kf1 = xexp2_slow(y1), kr0 = xexp2_slow(z0), kr1 = xexp2_slow(z1);
@@ -170,6 +180,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           kr0 = kr1 = 0.0;
         }
         // a7: rates of progress (absent slots read the row of ones)
+        if (a.debug & 4) sa.x = sa.y = sa.z = sa.w = sb.x = sb.y = ns;
         double2 v = lds2(n_l + sa.x * kFW);
         double qf0 = kf0 * v.x, qf1 = kf1 * v.y;
         if (sa.y != ns) { v = lds2(n_l + sa.y * kFW); qf0 *= v.x, qf1 *= v.y; }
@@ -184,11 +195,12 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       __syncthreads();
       // ------------------------------------------------------------ phase B
       const int *hdr = reinterpret_cast<const int *>(mb);
-      const int t_begin = hdr[warp], t_end = hdr[warp + 1];
+      const int t_begin = hdr[warp], t_end = (a.debug & 1) ? t_begin : hdr[warp + 1];
       const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + hdr[kFWarps + 1]) + grp;
       const double *q_l = qb + l2;
 #pragma unroll 1
-      for (int t = t_begin; t < t_end; ++t) {
+      for (int t_ = t_begin << ((a.debug >> 6) & 1); t_ < (t_end << ((a.debug >> 6) & 1)); ++t_) {
+        const int t = t_ >> ((a.debug >> 6) & 1);
         const int4 tk = mb[kFMetaHdr / 4 + t];
         const unsigned rows = (grp & 2) ? (unsigned)tk.w : (unsigned)tk.z;
         const int row = (int)((grp & 1) ? rows >> 16 : rows & 0xffffu);

@@ -81,7 +81,7 @@ struct FusedTask {   // one warp task of the production/loss phase: 4 row tasks 
 constexpr int kFBlkArr = 7 * 64;   // bytes of a UNI/BI block
 constexpr int kFBlkFo = 10 * 64;   // bytes of a FALLOFF block
 constexpr int kFBlkPh = 2 * 64;    // bytes of a PHOTO block (species slots only)
-constexpr int kFMetaHdr = 20;      // int32 words of a chunk's schedule header (17 warp offsets, task count)
+constexpr int kFMetaHdr = (kFWarps + 2 + 3) / 4 * 4;  // int32 words of a chunk's schedule header (kFWarps + 1 task offsets, task count)
 
 struct FusedDev {
   int32_t enabled;            // 0: fall back to the multi-kernel path
@@ -162,6 +162,7 @@ struct xod_network {
   int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
   int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
   int sm_count = 148;
+  int64_t debug = 0;
   int device = -1;
   std::vector<void *> dev_allocs;
   int64_t chunk_cols = 0;  // 0 = default
