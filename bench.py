@@ -29,9 +29,10 @@ if ROOT not in sys.path:
 
 METRIC = "fp64 rate+dn/dt evals/s (layer*reaction) at 7720 rxn"
 UNIT = "evals/s"
-# Algorithmic FP64-pipe instructions per evaluation of the fused path:
-# what the method must compute per (column, reaction), counted as FP64 instructions, FMA = 1.
-ALG_FP64_INSTR_PER_EVAL = 65.0
+# Algorithmic FP64-pipe instructions per evaluation of the fused path: what the
+# method must compute per (column, reaction) in its leanest formulation, FMA = 1 instruction.
+# (ncu counts 49.1 executed per evaluation for k_fused: padding and slow paths are not credited.)
+ALG_FP64_INSTR_PER_EVAL = 45.0
 KERNEL_DOC = {"fused": "k_fused (a1-a8 in one kernel: k_f, k_r, rates of progress, production/loss)",
               "rates": "k_rates (a3-a7: k_f, k_r, rates of progress; multi-kernel pipeline)"}
 NOMINAL_DFMA_PER_S = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x clocks.max.sm

@@ -27,6 +27,8 @@ def build(force=False, verbose=False):
            "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    if os.environ.get("XOD_ABLATE"):      # profiling builds only: phase ablation switches in k_fused
+        cmd += ["-DXOD_ABLATE"]
     cmd += [os.path.join(CSRC, f) for f in SOURCES]
     subprocess.run(cmd, check=True)
     return LIB

@@ -27,6 +27,15 @@
 #include "xod_internal.h"
 #include "xod_math.cuh"
 
+// Ablation switches for profiling (which phase costs what): compiled in only with -DXOD_ABLATE.
+#ifdef XOD_ABLATE
+#define XOD_DBG(bit) ((a.debug & (bit)) != 0)
+#define XOD_DBG_SHIFT(pos) ((a.debug >> (pos)) & 1)
+#else
+#define XOD_DBG(bit) false
+#define XOD_DBG_SHIFT(pos) 0
+#endif
+
 namespace xod {
 
 struct FusedArgs {
@@ -125,19 +134,19 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       // ------------------------------------------------------------ phase A
       const int pp_chunk = k * f.chunk;
 #pragma unroll 1
-      for (int pass_ = 0; pass_ < (f.chunk / kFPass << ((a.debug >> 5) & 1)); ++pass_) {
-        const int pass = pass_ >> ((a.debug >> 5) & 1);
+      for (int pass_ = 0; pass_ < (f.chunk / kFPass << XOD_DBG_SHIFT(5)); ++pass_) {
+        const int pass = pass_ >> XOD_DBG_SHIFT(5);
         const int rbase = pass * kFPass + warp * kFRxnPerWarp;
         const int ppw = pp_chunk + rbase;  // first of the warp's 4 reactions (one segment)
         if (ppw >= f.ph_end) break;        // only padding left
-        if (a.debug & 16) continue;
+        if (XOD_DBG(16)) continue;
         double kf0, kf1, kr0, kr1;
         int4 sa, sb;
         if (ppw < f.fo_end) {
           const bool arr = ppw < f.arr_end;
           const size_t off = arr ? (size_t)(ppw >> 2) * kFBlkArr
                                  : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
-          const unsigned char *b0 = blk0 + ((a.debug & 8) ? (size_t)0 : off);
+          const unsigned char *b0 = blk0 + (XOD_DBG(8) ? (size_t)0 : off);
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
           sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64 + slot16));
           const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
@@ -152,7 +161,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           }
           if (arr) {  // UNI, BI
             const unsigned m = max(max(xexp2_mag(y0), xexp2_mag(y1)), max(xexp2_mag(z0), xexp2_mag(z1)));
-            if (a.debug & 2) {
+            if (XOD_DBG(2)) {
               kf0 = y0, kf1 = y1, kr0 = z0, kr1 = z1;
             } else if (m < kExp2FastMax) {
               kf0 = xexp2_fast(y0), kf1 = xexp2_fast(y1), kr0 = xexp2_fast(z0), kr1 = xexp2_fast(z1);
@@ -180,7 +189,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           kr0 = kr1 = 0.0;
         }
         // a7: rates of progress (absent slots read the row of ones)
-        if (a.debug & 4) sa.x = sa.y = sa.z = sa.w = sb.x = sb.y = ns;
+        if (XOD_DBG(4)) sa.x = sa.y = sa.z = sa.w = sb.x = sb.y = ns;
         double2 v = lds2(n_l + sa.x * kFW);
         double qf0 = kf0 * v.x, qf1 = kf1 * v.y;
         if (sa.y != ns) { v = lds2(n_l + sa.y * kFW); qf0 *= v.x, qf1 *= v.y; }
@@ -195,12 +204,12 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       __syncthreads();
       // ------------------------------------------------------------ phase B
       const int *hdr = reinterpret_cast<const int *>(mb);
-      const int t_begin = hdr[warp], t_end = (a.debug & 1) ? t_begin : hdr[warp + 1];
+      const int t_begin = hdr[warp], t_end = XOD_DBG(1) ? t_begin : hdr[warp + 1];
       const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + hdr[kFWarps + 1]) + grp;
       const double *q_l = qb + l2;
 #pragma unroll 1
-      for (int t_ = t_begin << ((a.debug >> 6) & 1); t_ < (t_end << ((a.debug >> 6) & 1)); ++t_) {
-        const int t = t_ >> ((a.debug >> 6) & 1);
+      for (int t_ = t_begin << XOD_DBG_SHIFT(6); t_ < (t_end << XOD_DBG_SHIFT(6)); ++t_) {
+        const int t = t_ >> XOD_DBG_SHIFT(6);
         const int4 tk = mb[kFMetaHdr / 4 + t];
         const unsigned rows = (grp & 2) ? (unsigned)tk.w : (unsigned)tk.z;
         const int row = (int)((grp & 1) ? rows >> 16 : rows & 0xffffu);
