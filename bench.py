@@ -154,6 +154,21 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------- our arm
+def max_over_ranks(value, device="cpu"):
+    """The slowest rank's time decides (replicas only: no other exchange on the path)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(evals_per_rank, world, ms_step_max):
+    """Weak scaling: every rank processes its own replica of the batch; value = all evaluations / max time."""
+    return evals_per_rank * world / (ms_step_max * 1e-3)
+
+
 def event_time_ms(fn, reps, stream_sync):
     import torch
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -279,12 +294,9 @@ def run_ours(args):
     kt = h.timing_read()
     h.tune(binding.XOD_TUNE_TIMING, 0)
     clocks = sampler.stop(w0, w1)
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item()) / args.steps
+    ms_step = max_over_ranks(ms_total, "cuda") / args.steps
     evals_per_step = ncol * nr * world
-    value = evals_per_step / (ms_step * 1e-3)
+    value = whole_job_value(ncol * nr, world, ms_step)
 
     # ---- end to end through the host-buffer entry point (pinned host memory, copies timed)
     hT, hP, hJ, hn = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (atm.T, atm.P, atm.J, atm.n)]
@@ -301,10 +313,7 @@ def run_ours(args):
     e1.record()
     barrier()
     e2e_ms = max(e0.elapsed_time(e1), 0.0) / k2
-    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, "cuda")
     h2d = (2 + net.n_photo + ns) * ld * 8
     d2h = ns * ld * 8
 
