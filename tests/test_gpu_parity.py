@@ -327,3 +327,98 @@ def test_workspace_too_small_is_an_error(xod, network):
         h.source_fused(atm.ncol, atm.ncol - 1, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0,
                        workspace=G.workspace(h.source_fused_workspace_bytes(atm.ncol)))
     assert e.value.status == 1
+
+
+# ------------------------------------------------------------------------------- full sizes, sampled
+def _gather_columns(atm, cols):
+    """A compact atmosphere holding only the sampled columns (oracle input)."""
+    return atm.T[cols].copy(), atm.P[cols].copy(), atm.J[:, cols].copy(), atm.n[:, cols].copy()
+
+
+def test_full_size_config4_sampled_columns(xod, oracle, network):
+    """BASELINE config 4 at full size (256 x 150 = 38 400 columns) in the launch configuration
+    bench.py times (one xod_source_fused call), checked on sampled columns the oracle evaluates one
+    by one: tile edges, the first and last tile, random interior columns."""
+    net = network(4)
+    h = handle(xod, network, 4)
+    atm = atmosphere(4, net)
+    assert atm.ncol == 38400
+    ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+    d0 = G.empty(net.n_species, atm.ld)
+    h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    got = G.host(d0)
+    rng = np.random.default_rng(4)
+    cols = np.unique(np.concatenate([[0, 1, 15, 16, 17, 31, 32, atm.ncol - 17, atm.ncol - 16, atm.ncol - 1],
+                                     rng.integers(0, atm.ncol, size=54)]))
+    T, P, J, n = _gather_columns(atm, cols)
+    okf, okr = oracle.rate_coeffs(net, T, P, J)
+    want, wp, wl = oracle.source(net, okf, okr, n)
+    ok = G.finite_columns(okf, okr, want, wp, wl)
+    assert ok.sum() >= cols.size // 2
+    G.check_sum(got[:, cols], want, wp + wl, np.flatnonzero(ok), "full-size fused dn/dt (sampled)")
+    assert element_residual(net, got[:, cols], wp + wl, np.flatnonzero(ok)) <= 1e-13
+    # a property that holds at any size: columns whose inputs are finite give finite-or-inf results, never NaN
+    # unless an overflowed k_r met a zero density (inf x 0), which the oracle reproduces on the sampled columns
+    nan_cols = np.isnan(got[:, cols]).any(axis=0)
+    assert np.array_equal(nan_cols, np.isnan(want).any(axis=0))
+
+
+def test_full_size_config5_jacobian_sampled_columns(xod, oracle, network):
+    """BASELINE config 5 at full size (64 x 150 = 9 600 columns): rate coefficients, dn/dt and
+    Jacobian values, checked on sampled columns."""
+    net = network(5)
+    h = handle(xod, network, 5)
+    atm = atmosphere(5, net)
+    assert atm.ncol == 9600
+    nr, ns, ld = net.n_reactions, net.n_species, atm.ld
+    T, P, J, n = G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n)
+    kf, kr = G.empty(nr, ld), G.empty(nr, ld)
+    h.rate_coeffs(atm.ncol, ld, T, P, J, kf, kr, G.workspace(h.rate_coeffs_workspace_bytes(atm.ncol)))
+    jac = G.empty(h.nnz_jac, ld)
+    h.jacobian(atm.ncol, ld, kf, kr, n, jac)
+    d0 = G.empty(ns, ld)
+    h.source(atm.ncol, ld, kf, kr, n, d0, workspace=G.workspace(h.source_workspace_bytes(atm.ncol)))
+    cols = np.array([0, 31, 32, 4799, 9568, 9599])
+    Tc, Pc, Jc, nc = _gather_columns(atm, cols)
+    okf, okr = oracle.rate_coeffs(net, Tc, Pc, Jc)
+    G.check_k(G.host(kf)[:, cols], okf, "full-size k_f")
+    G.check_k(G.host(kr)[:, cols], okr, "full-size k_r")
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, nc, rp, col)
+    G.check_sum(G.host(jac)[:, cols], wj, sj, np.arange(cols.size), "full-size Jacobian (sampled)")
+    want, wp, wl = oracle.source(net, okf, okr, nc)
+    G.check_sum(G.host(d0)[:, cols], want, wp + wl, np.arange(cols.size), "full-size dn/dt (sampled)")
+
+
+def test_reaction_split_path_matches_single_pass(xod, oracle, network):
+    """Few columns: the chunks of a tile are split over several CTAs and combined in split order.
+    Forced splits must agree with the oracle like the automatic choice does."""
+    net = network(3)
+    atm = atmosphere(3, net)
+    want, wp, wl = oracle.source_from_state(net, atm.T, atm.P, atm.J, atm.n, atm.ncol)
+    for split in (1, 3, 31):
+        h = xod.Network(net, device=0)
+        h.tune(xod.XOD_TUNE_SPLIT, split)
+        ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+        d0 = G.empty(net.n_species, atm.ld)
+        h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+        G.check_sum(G.host(d0), want, wp + wl, np.arange(atm.ncol), "split %d" % split)
+        assert np.all(np.isnan(G.host(d0)[:, atm.ncol:]))
+        h.close()
+
+
+def test_many_thermo_breakpoints_fall_back_to_the_multi_kernel_path(xod, oracle, network):
+    """More than 31 distinct t_mid values: the fused single-kernel tables are disabled and
+    xod_source_fused runs the multi-kernel pipeline; results still match the oracle."""
+    import copy
+    net = copy.copy(network(2))
+    net.t_mid = 300.0 + 10.0 * np.arange(net.n_species)
+    h = xod.Network(net, device=0)
+    assert h.fused_info()["enabled"] == 0
+    atm = atmosphere(2, net)
+    want, wp, wl = oracle.source_from_state(net, atm.T, atm.P, atm.J, atm.n, atm.ncol)
+    ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+    d0 = G.empty(net.n_species, atm.ld)
+    h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    G.check_sum(G.host(d0), want, wp + wl, np.arange(atm.ncol), "fallback dn/dt")
+    h.close()
