@@ -207,27 +207,65 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       const int t_begin = hdr[warp], t_end = XOD_DBG(1) ? t_begin : hdr[warp + 1];
       const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + hdr[kFWarps + 1]) + grp;
       const double *q_l = qb + l2;
-#pragma unroll 1
-      for (int t_ = t_begin << XOD_DBG_SHIFT(6); t_ < (t_end << XOD_DBG_SHIFT(6)); ++t_) {
-        const int t = t_ >> XOD_DBG_SHIFT(6);
-        const int4 tk = mb[kFMetaHdr / 4 + t];
+      // two warp tasks in flight per iteration (their loads are independent): the dependent
+      // chain header -> entry -> q -> FMA is the latency that matters here, not the instruction count
+      auto row_of = [&](const int4 &tk) {
         const unsigned rows = (grp & 2) ? (unsigned)tk.w : (unsigned)tk.z;
-        const int row = (int)((grp & 1) ? rows >> 16 : rows & 0xffffu);
-        const unsigned *e = ent + tk.x;
-        double s0 = 0.0, s1 = 0.0;
-#pragma unroll 1
-        for (int st = 0; st < tk.y; ++st) {
-          const unsigned en = e[st * 4];
-          const double nu = __hiloint2double((int)(en & 0xffff0000u), 0);
-          const double2 qv = lds2(q_l + (en & 0xffffu) * kFW);
-          s0 = fma(nu, qv.x, s0), s1 = fma(nu, qv.y, s1);
-        }
+        return (int)((grp & 1) ? rows >> 16 : rows & 0xffffu);
+      };
+      auto add_row = [&](int row, double s0, double s1) {
         if (row != 0xffff) {
           double2 *dst = reinterpret_cast<double2 *>(acc_s + (size_t)row * kFW + l2);
           double2 cur = *dst;
           cur.x += s0, cur.y += s1;
           *dst = cur;
         }
+      };
+      int t = t_begin;
+#pragma unroll 1
+      for (; t + 1 < t_end; t += 2) {
+        const int4 ta = mb[kFMetaHdr / 4 + t], tb = mb[kFMetaHdr / 4 + t + 1];
+        const unsigned *ea = ent + ta.x, *eb = ent + tb.x;
+        double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+        const int nmin = min(ta.y, tb.y);
+        int st = 0;
+#pragma unroll 1
+        for (; st < nmin; ++st) {
+          const unsigned xa = ea[st * 4], xb = eb[st * 4];
+          const double2 qa = lds2(q_l + (xa & 0xffffu) * kFW), qc = lds2(q_l + (xb & 0xffffu) * kFW);
+          const double na = __hiloint2double((int)(xa & 0xffff0000u), 0), nb = __hiloint2double((int)(xb & 0xffff0000u), 0);
+          a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
+          b0 = fma(nb, qc.x, b0), b1 = fma(nb, qc.y, b1);
+        }
+#pragma unroll 1
+        for (int s2 = st; s2 < ta.y; ++s2) {
+          const unsigned xa = ea[s2 * 4];
+          const double2 qa = lds2(q_l + (xa & 0xffffu) * kFW);
+          const double na = __hiloint2double((int)(xa & 0xffff0000u), 0);
+          a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
+        }
+#pragma unroll 1
+        for (int s2 = st; s2 < tb.y; ++s2) {
+          const unsigned xb = eb[s2 * 4];
+          const double2 qc = lds2(q_l + (xb & 0xffffu) * kFW);
+          const double nb = __hiloint2double((int)(xb & 0xffff0000u), 0);
+          b0 = fma(nb, qc.x, b0), b1 = fma(nb, qc.y, b1);
+        }
+        add_row(row_of(ta), a0, a1);
+        add_row(row_of(tb), b0, b1);
+      }
+      if (t < t_end) {
+        const int4 ta = mb[kFMetaHdr / 4 + t];
+        const unsigned *ea = ent + ta.x;
+        double a0 = 0.0, a1 = 0.0;
+#pragma unroll 1
+        for (int st = 0; st < ta.y; ++st) {
+          const unsigned xa = ea[st * 4];
+          const double2 qa = lds2(q_l + (xa & 0xffffu) * kFW);
+          const double na = __hiloint2double((int)(xa & 0xffff0000u), 0);
+          a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
+        }
+        add_row(row_of(ta), a0, a1);
       }
     }
     __syncthreads();
