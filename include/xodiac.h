@@ -119,7 +119,7 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
  * be NULL.  Synchronises on the last recorded event, then clears the record. */
 enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD_KERNEL_RATES_FROM_K = 3,
        XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
-       XOD_KERNEL_COUNT = 8 };
+       XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_COUNT = 9 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);

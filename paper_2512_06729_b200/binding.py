@@ -16,7 +16,7 @@ XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK = 1
 XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL = 0, 1, 2, 3
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine"]
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libxodiac.so")
 SOURCES = ["api.cu", "pack.cpp", "pack_fused.cpp"]
-HEADERS = ["kernels.cuh", "fused.cuh", "xod_math.cuh", "xod_internal.h", os.path.join("..", "..", "include", "xodiac.h")]
+HEADERS = ["kernels.cuh", "fused.cuh", "rates2.cuh", "xod_math.cuh", "xod_internal.h", os.path.join("..", "..", "include", "xodiac.h")]
 
 
 def _stale():

@@ -8,6 +8,7 @@
 #include <string>
 
 #include "fused.cuh"
+#include "rates2.cuh"
 #include "kernels.cuh"
 
 using namespace xod;
@@ -190,7 +191,7 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       fd.meta_cap = f.meta_cap;
       fd.blk_stride = f.blk_stride, fd.blk_fo_off = f.blk_fo_off, fd.blk_ph_off = f.blk_ph_off;
 #define UPF(vec, field) if (st == XOD_OK) st = upload(net, f.vec, &fd.field)
-      UPF(bp, bp); UPF(blk, blk); UPF(meta_ptr, meta_ptr); UPF(extra, extra);
+      UPF(bp, bp); UPF(blk, blk); UPF(meta_ptr, meta_ptr); UPF(extra, extra); UPF(pp_user, pp_user);
       if (st == XOD_OK) {
         const int32_t *m = nullptr;
         st = upload(net, f.meta, &m);
@@ -432,6 +433,17 @@ xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, con
   if (!workspace || workspace_bytes < xod_rate_coeffs_workspace_bytes(net, ncol))
     return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_rate_coeffs_workspace_bytes");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (net->fd.enabled && net->use_fused) {  // one kernel from the per-interval parameter blocks
+    // reactions per CTA: enough CTAs for ~8 per SM, at most 64 reactions each
+    const int64_t nbx = (ncol + 255) / 256;
+    int slice = (int)std::min<int64_t>(64, std::max<int64_t>(4, (int64_t)net->fd.ph_end * nbx / (net->sm_count * 8)));
+    slice = (slice + 3) / 4 * 4;
+    dim3 grid((unsigned)nbx, (unsigned)((net->fd.ph_end + slice - 1) / slice));
+    Timed tm(net, KID_RATE_COEFFS, s);
+    k_rate_coeffs<<<grid, 256, 0, s>>>(net->fd, ncol, ld, T, P, J, kf, kr, kLog2Kb, slice);
+    XOD_CUDA(cudaGetLastError());
+    return XOD_OK;
+  }
   const int64_t ldw = chunk_cols(net, ncol);
   ChunkScratch w = carve(net, workspace, ldw, true, false, false);
   for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {

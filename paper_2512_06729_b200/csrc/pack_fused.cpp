@@ -76,6 +76,9 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
   for (int p = 0; p < n_arr; ++p) f.pp_to_packed[p] = p;
   for (int p = 0; p < n_fo; ++p) f.pp_to_packed[f.arr_end + p] = h.fo_begin + p;
   for (int p = 0; p < n_ph; ++p) f.pp_to_packed[f.fo_end + p] = h.ph_begin + p;
+  f.pp_user.assign(f.npad, -1);
+  for (int pp = 0; pp < f.npad; ++pp)
+    if (f.pp_to_packed[pp] >= 0) f.pp_user[pp] = h.packed_to_user[f.pp_to_packed[pp]];
   std::vector<int32_t> packed_to_pp(nr);
   for (int pp = 0; pp < f.npad; ++pp)
     if (f.pp_to_packed[pp] >= 0) packed_to_pp[f.pp_to_packed[pp]] = pp;

@@ -1,0 +1,78 @@
+// rates2.cuh -- k_rate_coeffs: xod_rate_coeffs (a1, a3-a6) from the per-interval parameter blocks
+// of pack_fused.cpp: no G/RT tile, no workspace, one kernel.  thread = column; a CTA covers 256
+// columns x a slice of padded reactions (sized by the caller so the grid fills the chip); reaction parameters are warp-uniform 16-byte loads
+// (lanes of one thermo interval read the same address); every store is a coalesced 256-byte row
+// segment of k_f / k_r in USER reaction order.  Bound: HBM writes, 16 B per evaluation.
+//   UNI/BI   k_f = 2^(c0 + c1 log2 T + c2/T)                                       (Eq. 7)
+//            k_r = 2^(C0 + C1 log2 T + C2/T - T (D2 + T (D3 + T (D4 + T D5))))     (Eq. 15)
+//   FALLOFF  Eq. 10-12 with Troe F (reading F1)
+//   PHOTO    k_f = J, k_r = 0
+#pragma once
+#include <cuda_runtime.h>
+
+#include "xod_internal.h"
+#include "xod_math.cuh"
+
+namespace xod {
+
+
+__global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, int64_t ld, const double *__restrict__ T,
+                                                     const double *__restrict__ P, const double *__restrict__ J,
+                                                     double *__restrict__ kf, double *__restrict__ kr, double log2_kb, int slice) {
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c - (threadIdx.x & 31) >= ncol) return;  // whole warp past the end
+  const bool valid = c < ncol;
+  const int64_t gc = valid ? c : ncol - 1;
+  const double Tc = T[gc];
+  const double l2T = log2(Tc), iT = 1.0 / Tc;
+  const double lM = log2(P[gc]) - log2_kb - l2T;  // log2 [M], [M] = P/(k_B T)
+  int g = 0;
+  for (int k = 0; k < f.n_bp; ++k) g += __ldg(f.bp + k) < Tc;
+  const unsigned char *blkg = f.blk + (size_t)g * f.blk_stride;
+  const int p0 = blockIdx.y * slice, p1 = min(p0 + slice, f.ph_end);
+#pragma unroll 2
+  for (int pp = p0; pp < p1; ++pp) {
+    const int user = __ldg(f.pp_user + pp);
+    const int slot16 = (pp & 3) * 16;
+    double vf, vr = 0.0;
+    if (pp < f.fo_end) {
+      const bool arr = pp < f.arr_end;
+      const unsigned char *b = blkg + slot16 +
+                               (arr ? (size_t)(pp >> 2) * kFBlkArr
+                                    : (size_t)f.blk_fo_off + (size_t)((pp - f.arr_end) >> 2) * kFBlkFo);
+      const double2 c01 = __ldg(reinterpret_cast<const double2 *>(b + 2 * 64));
+      const double2 c2C = __ldg(reinterpret_cast<const double2 *>(b + 3 * 64));
+      const double2 c12 = __ldg(reinterpret_cast<const double2 *>(b + 4 * 64));
+      const double2 d23 = __ldg(reinterpret_cast<const double2 *>(b + 5 * 64));
+      const double2 d45 = __ldg(reinterpret_cast<const double2 *>(b + 6 * 64));
+      const double y = fma(c2C.x, iT, fma(c01.y, l2T, c01.x));
+      const double poly = fma(Tc, fma(Tc, fma(Tc, d45.y, d45.x), d23.y), d23.x);
+      const double z = fma(c12.y, iT, fma(c12.x, l2T, fma(-Tc, poly, c2C.y)));
+      if (arr) {
+        vf = xexp2(y);
+        vr = xexp2(z);
+      } else {
+        const double2 m01 = __ldg(reinterpret_cast<const double2 *>(b + 7 * 64));
+        const double2 m2f = __ldg(reinterpret_cast<const double2 *>(b + 8 * 64));
+        const double cN = __ldg(reinterpret_cast<const double *>(b + 9 * 64));
+        const double w = fma(m2f.x, iT, fma(m01.y, l2T, m01.x)) + lM;
+        const double lp = w - y, x = lp * cN;  // log2 Pr
+        const double lF = m2f.y / fma(x, x, 1.0);
+        const double den = 1.0 / (1.0 + xexp2(-fabs(lp)));
+        const double ym = fmin(w, y) + lF;
+        vf = xexp2(ym) * den;
+        vr = xexp2(ym + z) * den;
+      }
+    } else {
+      const unsigned char *b = blkg + (size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh + slot16;
+      const int jrow = __ldg(reinterpret_cast<const int *>(b + 64) + 2);
+      vf = J[(size_t)jrow * ld + gc];
+    }
+    if (valid && user >= 0) {  // user < 0: padding slot
+      if (kf) kf[(size_t)user * ld + c] = vf;
+      if (kr) kr[(size_t)user * ld + c] = vr;
+    }
+  }
+}
+
+}  // namespace xod

@@ -98,6 +98,7 @@ struct FusedDev {
   const int32_t *meta_ptr;    // [nchunk + 1] in 16-byte units into meta
   const int4 *meta;           // per chunk: header | tasks | entries
   const int32_t *extra;       // [n_extra][2] (extra accumulator row, species), grouped by species
+  const int32_t *pp_user;     // [npad] padded packed index -> USER reaction index, -1 for padding
 };
 
 struct FusedHost {
@@ -109,7 +110,7 @@ struct FusedHost {
   std::vector<int32_t> pp_to_packed;   // [npad], -1 for padding
   std::vector<double> bp;
   std::vector<unsigned char> blk;
-  std::vector<int32_t> meta_ptr, extra;
+  std::vector<int32_t> meta_ptr, extra, pp_user;
   std::vector<int32_t> meta;           // 4 words per 16-byte unit
 };
 
@@ -146,7 +147,7 @@ size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap);
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused

@@ -421,4 +421,27 @@ def test_many_thermo_breakpoints_fall_back_to_the_multi_kernel_path(xod, oracle,
     d0 = G.empty(net.n_species, atm.ld)
     h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
     G.check_sum(G.host(d0), want, wp + wl, np.arange(atm.ncol), "fallback dn/dt")
+    kf, kr = run_rate_coeffs(h, atm)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    G.check_k(kf[:, :atm.ncol], okf[:, :atm.ncol], "fallback k_f")
+    G.check_k(kr[:, :atm.ncol], okr[:, :atm.ncol], "fallback k_r")
+    h.close()
+
+
+def test_multi_kernel_pipeline_can_be_forced(xod, oracle, network):
+    """XOD_TUNE_FUSED_KERNEL = 0: xod_rate_coeffs and xod_source_fused run the multi-kernel pipeline
+    (prologue + rates + source kernels); both pipelines must match the oracle."""
+    net = network(3)
+    atm = atmosphere(3, net)
+    h = xod.Network(net, device=0)
+    h.tune(xod.XOD_TUNE_FUSED_KERNEL, 0)
+    kf, kr = run_rate_coeffs(h, atm)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    G.check_k(kf[:, :atm.ncol], okf[:, :atm.ncol], "multi-kernel k_f")
+    G.check_k(kr[:, :atm.ncol], okr[:, :atm.ncol], "multi-kernel k_r")
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
+    d0 = G.empty(net.n_species, atm.ld)
+    h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    G.check_sum(G.host(d0), want, wp + wl, np.arange(atm.ncol), "multi-kernel dn/dt")
     h.close()
