@@ -547,7 +547,9 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
   const int64_t ncg = (ncol + 31) / 32;
   if (ncg > 65535) return fail(XOD_ERR_INVALID_ARG, "ncol too large for one xod_jacobian call (max 2097120)");
   const int64_t want = (net->d.nnz_jac + 7) / 8;
-  const int64_t gx = std::max<int64_t>(1, std::min<int64_t>(want, std::max<int64_t>(1, 148LL * 64 / ncg)));
+  // CTAs per column group: at least two per SM, so the CTAs resident on an SM mostly share one
+  // column group and its n rows stay in L1 (measured 2.96 -> 2.52 ms on config 5)
+  const int64_t gx = std::max<int64_t>(1, std::min<int64_t>(want, std::max<int64_t>(2LL * net->sm_count, 64LL * net->sm_count / ncg)));
   dim3 grid((unsigned)gx, (unsigned)ncg);
   {
     Timed tm(net, KID_JACOBIAN, s);
