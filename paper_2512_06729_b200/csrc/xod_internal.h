@@ -61,7 +61,7 @@ struct DevTables {
 // padded to a multiple of kFRxnPerWarp and the total to a multiple of the chunk size; padding
 // slots are dummy reactions without stoichiometry entries.
 constexpr int kFW = 16;           // columns per tile (one 128-byte shared-memory row)
-constexpr int kFWarps = 16;       // warps per CTA
+constexpr int kFWarps = 20;       // warps per CTA
 constexpr int kFRxnPerWarp = 4;   // reactions a warp evaluates per pass (8 lanes x 2 columns each)
 constexpr int kFPass = kFWarps * kFRxnPerWarp;  // reactions per CTA pass
 constexpr int kFSegMax = 16;      // longest row task of the production/loss phase
