@@ -152,10 +152,8 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
           const double y0 = fma(c2C.x, iT0, fma(c01.y, lT0, c01.x)), y1 = fma(c2C.x, iT1, fma(c01.y, lT1, c01.x));
           const double z0 = rev_eval(b0, slot16, c2C.y, T0, lT0, iT0);
-          double z1;
-          if (same_g) {
-            z1 = rev_eval(b0, slot16, c2C.y, T1, lT1, iT1);
-          } else {
+          double z1 = rev_eval(b0, slot16, c2C.y, T1, lT1, iT1);
+          if (!same_g) {  // the thread's two columns sit in different thermo intervals (rare): redo column 1
             const unsigned char *b1 = blk1 + off;
             z1 = rev_eval(b1, slot16, ldg2(b1 + 3 * 64 + slot16).y, T1, lT1, iT1);
           }
