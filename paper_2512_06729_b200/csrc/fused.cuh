@@ -1,6 +1,7 @@
 // fused.cuh -- k_fused: the whole source term a1-a8 of one column tile in ONE kernel (sm_100a).
 //
-// A CTA (16 warps) owns a tile of kFW = 16 consecutive columns and a range of reaction chunks.
+// A CTA (kFWarps = 20 warps, one per SM, persistent over tiles) owns a tile of kFW = 16
+// consecutive columns and a range of reaction chunks.
 // Shared memory holds, as [row][16] fp64 rows of 128 bytes (= all 32 banks, so gathers of whole
 // rows by different lane groups never conflict):
 //   n_s   [ns + 1]      number densities of the tile (+ a row of ones for absent species slots)
