@@ -155,9 +155,11 @@ xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, co
 xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
                         const double *kr, const double *n, double *jac, void *stream);
 
-/* ---- end-to-end convenience: the fused call on HOST buffers (pinned or pageable).  Copies
- * T, P, J, n to the device, runs xod_source_fused, copies dndt back and synchronises.  Device
- * staging buffers are owned by the network and grown on demand (not thread-safe on one network). */
+/* ---- end-to-end convenience: the fused call on HOST buffers (pinned for overlap; pageable works
+ * but serialises).  Columns are processed in chunks of one round of tiles per SM through three
+ * staging slots on private streams, so the H2D copy of the next chunk, the kernels of this one and
+ * the D2H copy of the previous one overlap; synchronises before returning.  Staging buffers and
+ * streams are owned by the network and grown on demand (not thread-safe on one network). */
 xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, const double *T,
                                  const double *P, const double *J, const double *n, double *dndt);
 

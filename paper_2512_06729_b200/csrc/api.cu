@@ -226,6 +226,8 @@ void xod_network_destroy(xod_network *net) {
   for (void *e : net->timing.pool) cudaEventDestroy(static_cast<cudaEvent_t>(e));
   for (void *p : net->dev_allocs) cudaFree(p);
   if (net->stage) cudaFree(net->stage);
+  for (void *hs : net->host_streams)
+    if (hs) cudaStreamDestroy(static_cast<cudaStream_t>(hs));
   delete net;
 }
 
@@ -566,29 +568,46 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
   if (ncol == 0) return XOD_OK;
   if (!T || !P || !n || !dndt) return fail(XOD_ERR_INVALID_ARG, "T, P, n or dndt is NULL");
   if (net->h.n_photo > 0 && !J) return fail(XOD_ERR_INVALID_ARG, "J is NULL but the network has photolysis reactions");
-  const size_t ns = net->h.ns, nph = net->h.n_photo, pitch = (size_t)ld * sizeof(double);
-  const size_t ws = xod_source_fused_workspace_bytes(net, ncol);
-  // staging layout: T | P | J | n | dndt | workspace
+  // Column-chunk pipeline over kHostSlots staging slots, one stream each: the H2D copy of chunk
+  // c + 1, the kernels of chunk c and the D2H copy of chunk c - 1 overlap (PCIe is full duplex).
+  // A chunk is one full round of column tiles on every SM (sm_count x 16 columns), so chunking
+  // costs the persistent kernel no tail.  Rows are strided in host memory: cudaMemcpy2DAsync.
+  const size_t ns = net->h.ns, nph = net->h.n_photo;
+  const int64_t cw = std::min<int64_t>(round_up(ncol, 32), (int64_t)net->sm_count * kFW);  // columns per chunk
+  const size_t ws = xod_source_fused_workspace_bytes(net, cw) + 256;
   const size_t rows = 2 + nph + 2 * ns;
-  const size_t need = rows * pitch + ws + 512;
+  const size_t slot_bytes = round_up((int64_t)(rows * cw * sizeof(double) + ws), 256);
+  const size_t need = slot_bytes * kHostSlots;
   if (net->stage_bytes < need) {
     if (net->stage) cudaFree(net->stage);
     net->stage = nullptr, net->stage_bytes = 0;
     XOD_CUDA(cudaMalloc(&net->stage, need));
     net->stage_bytes = need;
   }
-  double *dT = static_cast<double *>(net->stage), *dP = dT + ld, *dJ = dP + ld, *dn = dJ + nph * ld,
-         *dd = dn + ns * ld;
-  void *dws = dd + ns * ld;
-  cudaStream_t s = nullptr;
-  XOD_CUDA(cudaMemcpyAsync(dT, T, pitch, cudaMemcpyHostToDevice, s));
-  XOD_CUDA(cudaMemcpyAsync(dP, P, pitch, cudaMemcpyHostToDevice, s));
-  if (nph) XOD_CUDA(cudaMemcpyAsync(dJ, J, nph * pitch, cudaMemcpyHostToDevice, s));
-  XOD_CUDA(cudaMemcpyAsync(dn, n, ns * pitch, cudaMemcpyHostToDevice, s));
-  st = xod_source_fused(net, ncol, ld, dT, dP, dJ, dn, dd, nullptr, nullptr, dws, ws + 256, s);
-  if (st != XOD_OK) return st;
-  XOD_CUDA(cudaMemcpyAsync(dndt, dd, ns * pitch, cudaMemcpyDeviceToHost, s));
-  XOD_CUDA(cudaStreamSynchronize(s));
+  for (int i = 0; i < kHostSlots; ++i)
+    if (!net->host_streams[i]) {
+      cudaStream_t s = nullptr;
+      XOD_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+      net->host_streams[i] = s;
+    }
+  const size_t hp = (size_t)ld * sizeof(double), dp = (size_t)cw * sizeof(double);
+  int slot = 0;
+  for (int64_t c0 = 0; c0 < ncol; c0 += cw, slot = (slot + 1) % kHostSlots) {
+    const int64_t w = std::min(cw, ncol - c0);
+    const size_t wb = (size_t)w * sizeof(double);
+    cudaStream_t s = static_cast<cudaStream_t>(net->host_streams[slot]);
+    double *dT = reinterpret_cast<double *>(static_cast<char *>(net->stage) + slot_bytes * slot);
+    double *dP = dT + cw, *dJ = dP + cw, *dn = dJ + nph * cw, *dd = dn + ns * cw;
+    void *dws = dd + ns * cw;
+    XOD_CUDA(cudaMemcpyAsync(dT, T + c0, wb, cudaMemcpyHostToDevice, s));
+    XOD_CUDA(cudaMemcpyAsync(dP, P + c0, wb, cudaMemcpyHostToDevice, s));
+    if (nph) XOD_CUDA(cudaMemcpy2DAsync(dJ, dp, J + c0, hp, wb, nph, cudaMemcpyHostToDevice, s));
+    XOD_CUDA(cudaMemcpy2DAsync(dn, dp, n + c0, hp, wb, ns, cudaMemcpyHostToDevice, s));
+    st = xod_source_fused(net, w, cw, dT, dP, dJ, dn, dd, nullptr, nullptr, dws, ws, s);
+    if (st != XOD_OK) return st;
+    XOD_CUDA(cudaMemcpy2DAsync(dndt + c0, hp, dd, dp, wb, ns, cudaMemcpyDeviceToHost, s));
+  }
+  for (int i = 0; i < kHostSlots; ++i) XOD_CUDA(cudaStreamSynchronize(static_cast<cudaStream_t>(net->host_streams[i])));
   return XOD_OK;
 }
 

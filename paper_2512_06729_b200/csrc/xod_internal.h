@@ -156,6 +156,8 @@ struct TimingState {
 };
 }  // namespace xod
 
+constexpr int kHostSlots = 3;  // staging slots of xod_source_fused_host
+
 struct xod_network {
   xod::HostTables h;
   xod::DevTables d{};
@@ -170,5 +172,6 @@ struct xod_network {
   // staging for the *_host call
   void *stage = nullptr;
   size_t stage_bytes = 0;
+  void *host_streams[3] = {nullptr, nullptr, nullptr};  // cudaStream_t of the *_host pipeline slots
   mutable xod::TimingState timing;
 };

@@ -445,3 +445,19 @@ def test_multi_kernel_pipeline_can_be_forced(xod, oracle, network):
     h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
     G.check_sum(G.host(d0), want, wp + wl, np.arange(atm.ncol), "multi-kernel dn/dt")
     h.close()
+
+
+def test_host_entry_point_pipelines_column_chunks(xod, oracle, network):
+    """xod_source_fused_host on 5 000 columns: three chunks (2 x 2 368 + 264, the last one on the
+    reaction-split path) through the staging slots; checked on sampled columns of every chunk."""
+    from paper_2512_06729_b200 import synth
+    net = network(3)
+    h = handle(xod, network, 3)
+    atm = synth.make_atmosphere(91, net, 1, 5000)
+    out = np.full((net.n_species, atm.ld), np.nan)
+    h.source_fused_host(atm.ncol, atm.ld, atm.T, atm.P, atm.J, atm.n, out)
+    assert np.all(np.isfinite(out[:, :atm.ncol])) and np.all(np.isnan(out[:, atm.ncol:]))
+    cols = np.array([0, 15, 16, 2367, 2368, 2369, 4735, 4736, 4737, 4999])
+    T, P, J, n = _gather_columns(atm, cols)
+    want, wp, wl = oracle.source_from_state(net, T, P, J, n)
+    G.check_sum(out[:, cols], want, wp + wl, np.arange(cols.size), "host pipeline dn/dt (sampled)")
