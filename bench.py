@@ -35,7 +35,7 @@ UNIT = "evals/s"
 ALG_FP64_INSTR_PER_EVAL = 45.0
 KERNEL_DOC = {"fused": "k_fused (a1-a8 in one kernel: k_f, k_r, rates of progress, production/loss)",
               "rates": "k_rates (a3-a7: k_f, k_r, rates of progress; multi-kernel pipeline)"}
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_fused launch on config 4, from the ncu --set full
+# dram__bytes_read.sum + dram__bytes_write.sum of one step's k_fused work on config 4, from the ncu --set full
 # capture summarised in profiles/r01_k_fused_ncu.md (algorithmic: n 182 MB + J 190 MB in, dn/dt 182 MB out)
 NCU_DRAM_BYTES_PER_LAUNCH = {"fused": 379.0e6 + 155.2e6}
 NOMINAL_DFMA_PER_S = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x clocks.max.sm
@@ -335,7 +335,9 @@ def run_ours(args):
     peak = dfma * 2 / 1e12
     roofline = {"bound": "alu", "kernel": KERNEL_DOC.get(dom, dom), "achieved": achieved,
                 "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(dom) if args.workload == "config4" else None,
+                # ncu DRAM bytes of one step's k_fused work, spread over the launches the step makes
+                "traffic": (NCU_DRAM_BYTES_PER_LAUNCH[dom] * args.steps / max(k_n, 1)
+                            if args.workload == "config4" and dom in NCU_DRAM_BYTES_PER_LAUNCH else None),
                 "peak_source": "fp64 DFMA probe measured in this run (xod_probe_fp64_peak); nominal %.1f TFLOP/s"
                                % (NOMINAL_DFMA_PER_S * 2 / 1e12),
                 "alg_fp64_instr_per_eval": ALG_FP64_INSTR_PER_EVAL, "kernel_ms_avg": k_avg_ms, "kernel_launches": k_n,

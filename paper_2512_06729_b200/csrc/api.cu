@@ -378,9 +378,23 @@ int fused_split(const xod_network *net, int64_t ncol) {
   return (int)std::max<int64_t>(1, std::min<int64_t>(sp, net->h.f.nchunk));
 }
 
+// columns of the leading part that fills whole rounds of tiles on every SM (0: no such split).
+// The last partial round is launched separately with its chunks split over the idle SMs.
+int64_t fused_full_round_cols(const xod_network *net, int64_t ncol) {
+  const int64_t ntiles = (ncol + kFW - 1) / kFW, sm = net->sm_count;
+  if (net->force_split > 0 || ntiles <= sm || ntiles % sm == 0) return 0;
+  return ntiles / sm * sm * kFW;
+}
+
 xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T, const double *P,
                         const double *J, const double *n, double *dndt, void *workspace, cudaStream_t s) {
   const HostTables &h = net->h;
+  if (const int64_t c_full = fused_full_round_cols(net, ncol)) {  // columns are independent: two sub-ranges
+    xod_status st = launch_fused(net, c_full, ld, T, P, J, n, dndt, workspace, s);
+    if (st != XOD_OK) return st;
+    return launch_fused(net, ncol - c_full, ld, T + c_full, P + c_full, J ? J + c_full : J, n + c_full,
+                        dndt + c_full, workspace, s);
+  }
   FusedArgs a{};
   a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.J = J, a.n = n;
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
@@ -500,8 +514,9 @@ size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol) {
   if (!net || ncol < 0) return 0;
   size_t b = scratch_bytes(net, chunk_cols(net, ncol), true, true, true);
   if (net->h.f.enabled) {
-    const int ns_ = fused_split(net, ncol);
-    if (ns_ > 1) b = std::max(b, (size_t)ns_ * net->h.ns * (size_t)round_up(ncol, 32) * sizeof(double) + 256);
+    const int64_t rem = ncol - fused_full_round_cols(net, ncol);  // the part that may run split
+    const int ns_ = fused_split(net, rem);
+    if (ns_ > 1) b = std::max(b, (size_t)ns_ * net->h.ns * (size_t)round_up(rem, 32) * sizeof(double) + 256);
   }
   return b;
 }
