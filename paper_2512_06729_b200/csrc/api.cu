@@ -200,8 +200,10 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
 #undef UPF
       if (st == XOD_OK) {
         // the attribute is per function, not per network: always opt into the device maximum
-        cudaError_t ce = cudaFuncSetAttribute(k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t ce = cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                               (int)kFusedSmemMax);
+        if (ce == cudaSuccess)
+          ce = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
         if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_fused)");
       }
       int smc = 0;
@@ -386,17 +388,28 @@ int64_t fused_full_round_cols(const xod_network *net, int64_t ncol) {
   return ntiles / sm * sm * kFW;
 }
 
+// workspace bytes of the partial sums when k_fused splits the chunks of a tile over several CTAs
+size_t fused_partial_bytes(const xod_network *net, int64_t ncol) {
+  if (!net->h.f.enabled) return 0;
+  const int64_t rem = ncol - fused_full_round_cols(net, ncol);  // the part that may run split
+  const int ns_ = fused_split(net, rem);
+  return ns_ > 1 ? (size_t)ns_ * net->h.ns * (size_t)round_up(rem, 32) * sizeof(double) + 256 : 0;
+}
+
+// T, P, J given: xod_source_fused (coefficients evaluated in the kernel); kf, kr given: xod_source
 xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T, const double *P,
-                        const double *J, const double *n, double *dndt, void *workspace, cudaStream_t s) {
+                        const double *J, const double *kf, const double *kr, const double *n, double *dndt,
+                        void *workspace, cudaStream_t s) {
   const HostTables &h = net->h;
+  auto off = [](const double *p, int64_t c) { return p ? p + c : p; };
   if (const int64_t c_full = fused_full_round_cols(net, ncol)) {  // columns are independent: two sub-ranges
-    xod_status st = launch_fused(net, c_full, ld, T, P, J, n, dndt, workspace, s);
+    xod_status st = launch_fused(net, c_full, ld, T, P, J, kf, kr, n, dndt, workspace, s);
     if (st != XOD_OK) return st;
-    return launch_fused(net, ncol - c_full, ld, T + c_full, P + c_full, J ? J + c_full : J, n + c_full,
-                        dndt + c_full, workspace, s);
+    return launch_fused(net, ncol - c_full, ld, off(T, c_full), off(P, c_full), off(J, c_full), off(kf, c_full),
+                        off(kr, c_full), n + c_full, dndt + c_full, workspace, s);
   }
   FusedArgs a{};
-  a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.J = J, a.n = n;
+  a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.J = J, a.n = n, a.kf = kf, a.kr = kr;
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
   a.nsplit = fused_split(net, ncol);
   a.log2_kb = kLog2Kb;
@@ -409,7 +422,10 @@ xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const 
   const size_t smem = fused_smem_bytes(h.ns, h.f.n_acc, h.f.chunk, h.f.meta_cap);
   {
     Timed tm(net, KID_FUSED, s);
-    k_fused<<<grid, kFWarps * 32, smem, s>>>(net->fd, h.ns, a);
+    if (kf)
+      k_fused<true><<<grid, kFWarps * 32, smem, s>>>(net->fd, h.ns, a);
+    else
+      k_fused<false><<<grid, kFWarps * 32, smem, s>>>(net->fd, h.ns, a);
   }
   XOD_CUDA(cudaGetLastError());
   if (a.nsplit > 1) {
@@ -472,7 +488,7 @@ xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, con
 
 size_t xod_source_workspace_bytes(const xod_network *net, int64_t ncol) {
   if (!net || ncol < 0) return 0;
-  return scratch_bytes(net, chunk_cols(net, ncol), false, true, true);
+  return std::max(scratch_bytes(net, chunk_cols(net, ncol), false, true, true), fused_partial_bytes(net, ncol));
 }
 
 xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
@@ -488,6 +504,8 @@ xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const do
     return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_workspace_bytes");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const bool pl = prod != nullptr;
+  if (!pl && net->fd.enabled && net->use_fused && net->h.nr > 0)
+    return launch_fused(net, ncol, ld, nullptr, nullptr, nullptr, kf, kr, n, dndt, workspace, s);
   const int64_t ldw = chunk_cols(net, ncol);
   ChunkScratch w = carve(net, workspace, ldw, false, true, pl);
   for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {
@@ -512,13 +530,7 @@ xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const do
 
 size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol) {
   if (!net || ncol < 0) return 0;
-  size_t b = scratch_bytes(net, chunk_cols(net, ncol), true, true, true);
-  if (net->h.f.enabled) {
-    const int64_t rem = ncol - fused_full_round_cols(net, ncol);  // the part that may run split
-    const int ns_ = fused_split(net, rem);
-    if (ns_ > 1) b = std::max(b, (size_t)ns_ * net->h.ns * (size_t)round_up(rem, 32) * sizeof(double) + 256);
-  }
-  return b;
+  return std::max(scratch_bytes(net, chunk_cols(net, ncol), true, true, true), fused_partial_bytes(net, ncol));
 }
 
 xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
@@ -535,7 +547,8 @@ xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, co
     return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_fused_workspace_bytes");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   const bool pl = prod != nullptr;
-  if (!pl && net->fd.enabled && net->use_fused) return launch_fused(net, ncol, ld, T, P, J, n, dndt, workspace, s);
+  if (!pl && net->fd.enabled && net->use_fused)
+    return launch_fused(net, ncol, ld, T, P, J, nullptr, nullptr, n, dndt, workspace, s);
   const int64_t ldw = chunk_cols(net, ncol);
   ChunkScratch w = carve(net, workspace, ldw, true, true, pl);
   for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {

@@ -42,6 +42,7 @@ namespace xod {
 struct FusedArgs {
   int64_t ncol, ld;           // caller's columns and row pitch
   const double *T, *P, *J, *n;
+  const double *kf, *kr;      // FROMK only: stored coefficients [n_reactions][ld]
   double *out;                // nsplit == 1: dndt [ns][ld]; else partial sums [nsplit][ns][ldp]
   int64_t ldp;                // pitch of the partial sums
   int32_t ntiles, nsplit;
@@ -67,6 +68,16 @@ __device__ __forceinline__ double rev_eval(const unsigned char *blk, int slot16,
   return fma(c12.y, invT, fma(c12.x, l2T, fma(-T, poly, c0r)));
 }
 
+// FROMK = false: xod_source_fused (coefficients evaluated here, a1-a8).
+// FROMK = true : xod_source (a7-a8): k_f, k_r are read from the caller's arrays (USER reaction order).
+// byte offset of the parameter block (4 reactions) that holds padded reaction pp, inside an interval
+__device__ __forceinline__ size_t block_offset(const FusedDev &f, int pp) {
+  if (pp < f.arr_end) return (size_t)(pp >> 2) * kFBlkArr;
+  if (pp < f.fo_end) return (size_t)f.blk_fo_off + (size_t)((pp - f.arr_end) >> 2) * kFBlkFo;
+  return (size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh;
+}
+
+template <bool FROMK>
 __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, FusedArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   double *n_s = reinterpret_cast<double *>(smem_raw);
@@ -92,7 +103,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
     // ---- a1: column scalars (idle columns of a ragged tile reuse the last valid column)
     if (tid < kFW) {
       const int64_t gc = min(col0 + tid, a.ncol - 1);
-      const double Tc = a.T[gc], Pc = a.P[gc];
+      const double Tc = FROMK ? 1000.0 : a.T[gc], Pc = FROMK ? 1.0e6 : a.P[gc];
       const double l2T = log2(Tc);
       cT[tid] = Tc, cL2T[tid] = l2T, cInvT[tid] = 1.0 / Tc;
       cLM[tid] = log2(Pc) - a.log2_kb - l2T;  // log2 [M], [M] = P/(k_B T)
@@ -143,7 +154,16 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
         if (XOD_DBG(16)) continue;
         double kf0, kf1, kr0, kr1;
         int4 sa, sb;
-        if (ppw < f.fo_end) {
+        if (FROMK) {
+          const int pp = ppw + grp;
+          const unsigned char *b0 = blk0 + block_offset(f, pp) + slot16;
+          sa = __ldg(reinterpret_cast<const int4 *>(b0));
+          sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64));
+          const int user = max(__ldg(f.pp_user + pp), 0);  // padding slots read row 0 (their q is never used)
+          const int64_t gc0 = min(col0 + l2, a.ncol - 1), gc1 = min(col0 + l2 + 1, a.ncol - 1);
+          const double *kfr = a.kf + (size_t)user * a.ld, *krr = a.kr + (size_t)user * a.ld;
+          kf0 = __ldg(kfr + gc0), kf1 = __ldg(kfr + gc1), kr0 = __ldg(krr + gc0), kr1 = __ldg(krr + gc1);
+        } else if (ppw < f.fo_end) {
           const bool arr = ppw < f.arr_end;
           const size_t off = arr ? (size_t)(ppw >> 2) * kFBlkArr
                                  : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
