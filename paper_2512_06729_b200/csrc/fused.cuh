@@ -153,12 +153,11 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
         if (ppw >= f.ph_end) break;        // only padding left
         if (XOD_DBG(16)) continue;
         double kf0, kf1, kr0, kr1;
-        int4 sa, sb;
+        int4 sa;  // species slots as 16-bit indices: r0 r1 | r2 p0 | p1 p2 | J row
         if (FROMK) {
           const int pp = ppw + grp;
           const unsigned char *b0 = blk0 + block_offset(f, pp) + slot16;
           sa = __ldg(reinterpret_cast<const int4 *>(b0));
-          sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64));
           const int user = max(__ldg(f.pp_user + pp), 0);  // padding slots read row 0 (their q is never used)
           const int64_t gc0 = min(col0 + l2, a.ncol - 1), gc1 = min(col0 + l2 + 1, a.ncol - 1);
           const double *kfr = a.kf + (size_t)user * a.ld, *krr = a.kr + (size_t)user * a.ld;
@@ -169,7 +168,6 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
                                  : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
           const unsigned char *b0 = blk0 + (XOD_DBG(8) ? (size_t)0 : off);
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
-          sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64 + slot16));
           const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
           const double y0 = fma(c2C.x, iT0, fma(c01.y, lT0, c01.x)), y1 = fma(c2C.x, iT1, fma(c01.y, lT1, c01.x));
           const double z0 = rev_eval(b0, slot16, c2C.y, T0, lT0, iT0);
@@ -203,20 +201,20 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
         } else {                  // PHOTO
           const unsigned char *b0 = f.blk + (size_t)f.blk_ph_off + (size_t)((ppw - f.fo_end) >> 2) * kFBlkPh;
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
-          sb = __ldg(reinterpret_cast<const int4 *>(b0 + 64 + slot16));
-          kf0 = a.J[(size_t)sb.z * a.ld + gc0], kf1 = a.J[(size_t)sb.z * a.ld + gc1];
+          kf0 = a.J[(size_t)sa.w * a.ld + gc0], kf1 = a.J[(size_t)sa.w * a.ld + gc1];
           kr0 = kr1 = 0.0;
         }
         // a7: rates of progress (absent slots read the row of ones)
-        if (XOD_DBG(4)) sa.x = sa.y = sa.z = sa.w = sb.x = sb.y = ns;
-        double2 v = lds2(n_l + sa.x * kFW);
+        const int r0 = sa.x & 0xffff, r1 = (unsigned)sa.x >> 16, r2 = sa.y & 0xffff;
+        const int p0 = (unsigned)sa.y >> 16, p1 = sa.z & 0xffff, p2 = (unsigned)sa.z >> 16;
+        double2 v = lds2(n_l + r0 * kFW);
         double qf0 = kf0 * v.x, qf1 = kf1 * v.y;
-        if (sa.y != ns) { v = lds2(n_l + sa.y * kFW); qf0 *= v.x, qf1 *= v.y; }
-        if (sa.z != ns) { v = lds2(n_l + sa.z * kFW); qf0 *= v.x, qf1 *= v.y; }
-        v = lds2(n_l + sa.w * kFW);
+        if (r1 != ns) { v = lds2(n_l + r1 * kFW); qf0 *= v.x, qf1 *= v.y; }
+        if (r2 != ns) { v = lds2(n_l + r2 * kFW); qf0 *= v.x, qf1 *= v.y; }
+        v = lds2(n_l + p0 * kFW);
         double qr0 = kr0 * v.x, qr1 = kr1 * v.y;
-        if (sb.x != ns) { v = lds2(n_l + sb.x * kFW); qr0 *= v.x, qr1 *= v.y; }
-        if (sb.y != ns) { v = lds2(n_l + sb.y * kFW); qr0 *= v.x, qr1 *= v.y; }
+        if (p1 != ns) { v = lds2(n_l + p1 * kFW); qr0 *= v.x, qr1 *= v.y; }
+        if (p2 != ns) { v = lds2(n_l + p2 * kFW); qr0 *= v.x, qr1 *= v.y; }
         *reinterpret_cast<double2 *>(qb + (size_t)(rbase + grp) * kFW + l2) = make_double2(qf0 - qr0, qf1 - qr1);
       }
       cp_async_wait_all();

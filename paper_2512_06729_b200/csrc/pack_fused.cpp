@@ -58,7 +58,7 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
   std::sort(f.bp.begin(), f.bp.end());
   f.bp.erase(std::unique(f.bp.begin(), f.bp.end()), f.bp.end());
   f.n_bp = (int32_t)f.bp.size();
-  if (f.n_bp + 1 > kFMaxIntervals) return;
+  if (f.n_bp + 1 > kFMaxIntervals || ns >= 0xffff) return;
   std::vector<int> bp_of(ns);
   for (int i = 0; i < ns; ++i)
     bp_of[i] = (int)(std::lower_bound(f.bp.begin(), f.bp.end(), h.tmid[i]) - f.bp.begin());
@@ -136,7 +136,9 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
           v[10] = h.l0[fo], v[11] = h.l1[fo], v[12] = h.l2[fo], v[13] = h.fcl[fo], v[14] = h.cN[fo];
         }
       }
-      std::memcpy(blk + 0 * 64 + slot * 16, sp8, 16);
+      // unit 0: the six species slots as 16-bit indices (r0 r1 | r2 p0 | p1 p2) and the J row; unit 1 spare
+      const int32_t packed[4] = {sp8[0] | (sp8[1] << 16), sp8[2] | (sp8[3] << 16), sp8[4] | (sp8[5] << 16), sp8[6]};
+      std::memcpy(blk + 0 * 64 + slot * 16, packed, 16);
       std::memcpy(blk + 1 * 64 + slot * 16, sp8 + 4, 16);
       const int npair = seg == 0 ? 5 : seg == 1 ? 8 : 0;
       for (int u = 0; u < npair; ++u) std::memcpy(blk + (2 + u) * 64 + slot * 16, v + 2 * u, 16);

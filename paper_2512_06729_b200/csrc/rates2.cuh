@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, i
       }
     } else {
       const unsigned char *b = blkg + (size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh + slot16;
-      const int jrow = __ldg(reinterpret_cast<const int *>(b + 64) + 2);
+      const int jrow = __ldg(reinterpret_cast<const int *>(b) + 3);
       vf = J[(size_t)jrow * ld + gc];
     }
     if (valid && user >= 0) {  // user < 0: padding slot
