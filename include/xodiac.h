@@ -105,6 +105,11 @@ xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int
  * production/loss warp tasks, padded production/loss entries, bytes of the reverse-coefficient table */
 xod_status xod_network_fused_info(const xod_network *net, int64_t *info);
 
+/* host-only consistency check of the internal tables of the fused path (decoded as the kernel
+ * decodes them): every source-CSR entry scheduled exactly once, no accumulator row shared by two
+ * row tasks of a chunk, species slots intact.  XOD_OK, or XOD_ERR_INVALID_ARG with xod_last_error. */
+xod_status xod_network_selfcheck(const xod_network *net);
+
 /* ---- tuning knobs (optional; defaults are chosen for B200) */
 enum {
   XOD_TUNE_CHUNK_COLS = 0, /* columns per pipeline chunk of the fused source call (0 = default) */

@@ -25,7 +25,7 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_network_jac_pattern", "xod_network_tune", "xod_thermo",
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
-           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info"]
+           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck"]
 
 
 class XodError(RuntimeError):
@@ -152,6 +152,9 @@ class Network:
         _check(lib().xod_network_fused_info(self._h, v))
         keys = ("enabled", "chunk", "nchunk", "n_acc", "n_bp", "smem_bytes", "npad", "tasks", "entries", "rev_bytes")
         return dict(zip(keys, [int(x) for x in v]))
+
+    def selfcheck(self):
+        _check(lib().xod_network_selfcheck(self._h))
 
     def tune(self, knob, value):
         _check(lib().xod_network_tune(self._h, C.c_int32(knob), C.c_int64(value)))

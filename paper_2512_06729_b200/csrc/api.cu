@@ -285,6 +285,13 @@ xod_status xod_network_fused_info(const xod_network *net, int64_t *info) {
   return XOD_OK;
 }
 
+xod_status xod_network_selfcheck(const xod_network *net) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  std::string err;
+  if (!check_fused(net->h, err)) return fail(XOD_ERR_INVALID_ARG, err);
+  return XOD_OK;
+}
+
 xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
   if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
   if (knob == XOD_TUNE_CHUNK_COLS) {

@@ -243,3 +243,104 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
 }
 
 }  // namespace xod
+
+namespace xod {
+
+// Host-only self-check of the fused-path tables, decoding them exactly as k_fused does:
+//  * every (species, reaction, nu) entry of the source CSR appears exactly once in the chunk
+//    schedules, under its own species' accumulator row or one of that species' extra rows;
+//  * no accumulator row is written by two row tasks of one chunk (the atomic-free guarantee);
+//  * entry offsets, step counts and q-row indices stay inside their chunk;
+//  * the species slots and photolysis rows stored in the parameter blocks match the packed tables.
+// Returns true when consistent; otherwise err names the first violation.
+bool check_fused(const HostTables &h, std::string &err) {
+  const FusedHost &f = h.f;
+  if (!f.enabled) return true;
+  const int ns = h.ns;
+  auto fail = [&](const std::string &m) { err = "fused tables: " + m; return false; };
+  std::vector<int32_t> row_species(f.n_acc, -1);
+  for (int i = 0; i < ns; ++i) row_species[i] = i;
+  for (size_t x = 0; x + 1 < f.extra.size(); x += 2) {
+    if (f.extra[x] < ns || f.extra[x] >= f.n_acc || f.extra[x + 1] < 0 || f.extra[x + 1] >= ns) return fail("bad extra row");
+    row_species[f.extra[x]] = f.extra[x + 1];
+  }
+  for (int r = ns; r < f.n_acc; ++r)
+    if (row_species[r] < 0) return fail("unmapped extra row");
+  // expected multiset of (species, padded reaction, nu)
+  std::vector<int32_t> packed_to_pp(h.nr, -1);
+  for (int pp = 0; pp < f.npad; ++pp)
+    if (f.pp_to_packed[pp] >= 0) packed_to_pp[f.pp_to_packed[pp]] = pp;
+  std::vector<int64_t> want, got;
+  auto key = [&](int sp, int pp, int nu) { return ((int64_t)sp * f.npad + pp) * 8 + (nu + 4); };
+  for (int i = 0; i < ns; ++i)
+    for (int64_t e = h.src_ptr[i]; e < h.src_ptr[i + 1]; ++e)
+      want.push_back(key(i, packed_to_pp[h.src_rxn_packed[e]], h.src_nu[e]));
+  for (int k = 0; k < f.nchunk; ++k) {
+    const int32_t *blob = &f.meta[(size_t)f.meta_ptr[k] * 4];
+    const int64_t blob_words = ((int64_t)f.meta_ptr[k + 1] - f.meta_ptr[k]) * 4;
+    if (blob_words / 4 > f.meta_cap) return fail("schedule larger than meta_cap");
+    const int nt = blob[kFWarps + 1];
+    if (blob[0] != 0 || blob[kFWarps] != nt) return fail("bad warp offsets");
+    const int32_t *tasks = blob + kFMetaHdr;
+    const int32_t *ent = tasks + 4 * nt;
+    const int64_t nent = blob_words - kFMetaHdr - 4 * nt;
+    std::vector<char> row_used(f.n_acc, 0);
+    for (int w = 0; w < kFWarps; ++w) {
+      if (blob[w] > blob[w + 1]) return fail("warp offsets not monotone");
+      for (int t = blob[w]; t < blob[w + 1]; ++t) {
+        const int32_t off = tasks[4 * t], nsteps = tasks[4 * t + 1];
+        if (off < 0 || nsteps < 0 || nsteps > kFSegMax || (int64_t)off + 4 * nsteps > nent) return fail("task out of range");
+        for (int g = 0; g < 4; ++g) {
+          const uint32_t rows = (uint32_t)tasks[4 * t + 2 + (g >> 1)];
+          const int row = (g & 1) ? rows >> 16 : rows & 0xffffu;
+          for (int st = 0; st < nsteps; ++st) {
+            const uint32_t en = (uint32_t)ent[off + st * 4 + g];
+            const int rloc = en & 0xffffu;
+            uint64_t bits = (uint64_t)(en & 0xffff0000u) << 32;
+            double nu;
+            std::memcpy(&nu, &bits, 8);
+            if (rloc > f.chunk) return fail("q row beyond the chunk");
+            if (rloc == f.chunk) {
+              if (nu != 0.0) return fail("padding entry with nonzero nu");
+              continue;
+            }
+            if (row == 0xffff) return fail("entry under an idle lane group");
+            if (nu != std::floor(nu) || std::fabs(nu) > 3 || nu == 0.0) return fail("bad nu encoding");
+            got.push_back(key(row_species[row], k * f.chunk + rloc, (int)nu));
+          }
+          if (row != 0xffff) {
+            if (row >= f.n_acc) return fail("accumulator row out of range");
+            if (row_used[row]) return fail("accumulator row written by two row tasks of one chunk");
+            row_used[row] = 1;
+          }
+        }
+      }
+    }
+  }
+  std::sort(want.begin(), want.end());
+  std::sort(got.begin(), got.end());
+  if (want != got) return fail("schedule entries differ from the source CSR");
+  // parameter blocks: species slots and J rows, every interval
+  for (int g = 0; g <= f.n_bp; ++g)
+    for (int pp = 0; pp < f.ph_end; ++pp) {
+      const int seg = pp < f.arr_end ? 0 : pp < f.fo_end ? 1 : 2;
+      const int first = seg == 0 ? 0 : seg == 1 ? f.arr_end : f.fo_end;
+      const int64_t off = seg == 0 ? 0 : seg == 1 ? f.blk_fo_off : f.blk_ph_off;
+      const int bsz = seg == 0 ? kFBlkArr : seg == 1 ? kFBlkFo : kFBlkPh;
+      const unsigned char *blk = &f.blk[(size_t)g * f.blk_stride + off + (size_t)((pp - first) / kFRxnPerWarp) * bsz];
+      int32_t u[4];
+      std::memcpy(u, blk + ((pp - first) % kFRxnPerWarp) * 16, 16);
+      const int p = f.pp_to_packed[pp];
+      const int slots[6] = {u[0] & 0xffff, (int)((uint32_t)u[0] >> 16), u[1] & 0xffff, (int)((uint32_t)u[1] >> 16),
+                            u[2] & 0xffff, (int)((uint32_t)u[2] >> 16)};
+      for (int a = 0; a < 6; ++a) {
+        const int expect = p >= 0 && h.sp[(size_t)p * 6 + a] >= 0 ? h.sp[(size_t)p * 6 + a] : ns;
+        if (slots[a] != expect) return fail("species slot mismatch in a parameter block");
+      }
+      if (p >= h.ph_begin && u[3] != h.photo_row[p - h.ph_begin]) return fail("J row mismatch in a parameter block");
+      if (u[3] < 0 || (h.n_photo > 0 && u[3] >= h.n_photo) ) return fail("J row out of range");
+    }
+  return true;
+}
+
+}  // namespace xod

@@ -139,6 +139,8 @@ struct HostTables {
 xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &err);
 // pack_fused.cpp: tables of the fused path for a given chunk size (0 = does not fit: disabled)
 void pack_fused(const xod_network_desc *d, HostTables &h, int chunk);
+// host-only consistency check of the fused-path tables (pack_fused.cpp)
+bool check_fused(const HostTables &h, std::string &err);
 // shared-memory bytes k_fused needs for these tables
 size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap);
 

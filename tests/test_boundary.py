@@ -99,3 +99,25 @@ def test_charge_as_an_element_and_padding_anywhere(built, oracle):
     h = binding.Network(net, device=-1)
     assert np.array_equal(h.source_csr()[1], oracle.source_csr(net)[1])
     assert np.array_equal(h.jac_pattern()[1], oracle.jac_pattern(net)[1])
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_fused_path_tables_are_consistent(built, network, cfg):
+    """Host-side check of the single-kernel path's tables, decoded as the kernel decodes them: every
+    source-CSR entry is scheduled exactly once, no accumulator row is shared by two row tasks of a
+    chunk (the atomic-free guarantee), species slots and J rows survive the packing."""
+    net = network(cfg)
+    h = binding.Network(net, device=-1)
+    info = h.fused_info()
+    assert info["enabled"] == 1 and info["smem_bytes"] <= 227 * 1024
+    assert info["chunk"] % 80 == 0 and info["npad"] == info["chunk"] * info["nchunk"] >= net.n_reactions
+    h.selfcheck()
+
+
+def test_fused_path_disabled_for_many_thermo_intervals(built, network):
+    import copy
+    net = copy.copy(network(2))
+    net.t_mid = 300.0 + 10.0 * np.arange(net.n_species)
+    h = binding.Network(net, device=-1)
+    assert h.fused_info()["enabled"] == 0
+    h.selfcheck()
