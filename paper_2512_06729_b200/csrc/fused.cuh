@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           const bool arr = ppw < f.arr_end;
           const size_t off = arr ? (size_t)(ppw >> 2) * kFBlkArr
                                  : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
-          const unsigned char *b0 = blk0 + (XOD_DBG(8) ? (size_t)0 : off);
+          const unsigned char *b0 = blk0 + off;
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
           const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
           const double y0 = fma(c2C.x, iT0, fma(c01.y, lT0, c01.x)), y1 = fma(c2C.x, iT1, fma(c01.y, lT1, c01.x));
