@@ -105,6 +105,18 @@ xod_status xod_network_jac_pattern(const xod_network *net, int64_t *row_ptr, int
  * production/loss warp tasks, padded production/loss entries, bytes of the reverse-coefficient table */
 xod_status xod_network_fused_info(const xod_network *net, int64_t *info);
 
+/* host-only view of the fused path's parameter blocks for one thermo interval (0 .. breakpoints), for
+ * tests of the packer's arithmetic.  Arrays of info[6] = npad padded reactions: user_rxn (-1 = padding
+ * slot), kind (0 UNI/BI, 1 FALLOFF, 2 PHOTO, 3 padding), coef [npad][16] =
+ * c0 c1 c2 | C0 C1 C2 D2 D3 D4 D5 | l0 l1 l2 log2Fc cN | 0  with
+ *   log2 k_f (or log2 k_inf) = c0 + c1 log2 T + c2/T                                        (Eq. 7, 11)
+ *   C0 + C1 log2 T + C2/T - T (D2 + T (D3 + T (D4 + T D5))) = log2 k_r (UNI/BI) or log2 (k_r/k_f) (FALLOFF)
+ *   log2 k0 = l0 + l1 log2 T + l2/T                                                           (Eq. 10)
+ * breakpoints [info[4]]: the sorted distinct t_mid values; a column with T is in interval #{bp < T}.
+ * Any output may be NULL. */
+xod_status xod_network_fused_params(const xod_network *net, int32_t interval, int32_t *user_rxn, int32_t *kind,
+                                    double *coef, double *breakpoints);
+
 /* host-only consistency check of the internal tables of the fused path (decoded as the kernel
  * decodes them): every source-CSR entry scheduled exactly once, no accumulator row shared by two
  * row tasks of a chunk, species slots intact.  XOD_OK, or XOD_ERR_INVALID_ARG with xod_last_error. */

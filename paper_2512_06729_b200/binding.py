@@ -25,7 +25,7 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_network_jac_pattern", "xod_network_tune", "xod_thermo",
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
-           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck"]
+           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params"]
 
 
 class XodError(RuntimeError):
@@ -152,6 +152,16 @@ class Network:
         _check(lib().xod_network_fused_info(self._h, v))
         keys = ("enabled", "chunk", "nchunk", "n_acc", "n_bp", "smem_bytes", "npad", "tasks", "entries", "rev_bytes")
         return dict(zip(keys, [int(x) for x in v]))
+
+    def fused_params(self, interval):
+        """(user_rxn [npad], kind [npad], coef [npad][16], breakpoints) of one thermo interval."""
+        info = self.fused_info()
+        user = np.zeros(info["npad"], dtype=np.int32)
+        kind = np.zeros(info["npad"], dtype=np.int32)
+        coef = np.zeros((info["npad"], 16))
+        bp = np.zeros(info["n_bp"])
+        _check(lib().xod_network_fused_params(self._h, C.c_int32(interval), _hp(user), _hp(kind), _hp(coef), _hp(bp)))
+        return user, kind, coef, bp
 
     def selfcheck(self):
         _check(lib().xod_network_selfcheck(self._h))

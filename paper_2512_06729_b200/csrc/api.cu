@@ -285,6 +285,32 @@ xod_status xod_network_fused_info(const xod_network *net, int64_t *info) {
   return XOD_OK;
 }
 
+xod_status xod_network_fused_params(const xod_network *net, int32_t interval, int32_t *user_rxn, int32_t *kind,
+                                    double *coef, double *breakpoints) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  const HostTables &h = net->h;
+  const FusedHost &f = h.f;
+  if (!f.enabled) return fail(XOD_ERR_INVALID_ARG, "the fused-path tables are disabled for this network");
+  if (interval < 0 || interval > f.n_bp) return fail(XOD_ERR_INVALID_ARG, "interval out of range");
+  if (breakpoints) std::memcpy(breakpoints, f.bp.data(), f.bp.size() * sizeof(double));
+  for (int pp = 0; pp < f.npad; ++pp) {
+    if (user_rxn) user_rxn[pp] = f.pp_user[pp];
+    const int seg = pp < f.arr_end ? 0 : pp < f.fo_end ? 1 : pp < f.ph_end ? 2 : 3;
+    if (kind) kind[pp] = seg;
+    if (!coef) continue;
+    double *out = coef + (size_t)pp * 16;
+    for (int k = 0; k < 16; ++k) out[k] = 0.0;
+    if (seg >= 2) continue;
+    const int first = seg == 0 ? 0 : f.arr_end;
+    const int64_t off = seg == 0 ? 0 : f.blk_fo_off;
+    const int bsz = seg == 0 ? kFBlkArr : kFBlkFo;
+    const unsigned char *blk = &f.blk[(size_t)interval * f.blk_stride + off + (size_t)((pp - first) / kFRxnPerWarp) * bsz];
+    const int slot = (pp - first) % kFRxnPerWarp, npair = seg == 0 ? 5 : 8;
+    for (int u = 0; u < npair; ++u) std::memcpy(out + 2 * u, blk + (2 + u) * 64 + slot * 16, 16);
+  }
+  return XOD_OK;
+}
+
 xod_status xod_network_selfcheck(const xod_network *net) {
   if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
   std::string err;
