@@ -207,3 +207,33 @@ def test_reverse_coefficient_saturates_like_ieee(oracle, oracle_f64):
     assert kr[0, 0] == pytest.approx(float(np.longdouble(1e-40) * np.exp(np.longdouble(800.0))), rel=1e-13)
     assert 2.72e307 < kr[0, 0] < 2.73e307       # e^800 = 2.7264e347
     assert np.isinf(kr[0, 1])
+
+
+def test_table1_phosphorus_network_equilibrium_constant(oracle):
+    """The only element-balanced reaction among the paper's Table 1 species, 2 P2O <=> P2O2 + 2 P(2D)
+    (SURVEY section 4), with the PRINTED coefficients: K_c from the oracle's
+    k_f/k_r against G/RT evaluated here from the printed line-671 formula with exact fractions.
+    dnu = 3 - 2 = +1, so K_c = exp(-dG/RT) * P0/(k_B T) [cm^-3]."""
+    from fractions import Fraction
+    rows = load_table1()
+    names = ["P2O", "P2O2", "P2D"]
+    lo = np.array([rows[n + "_lo"] for n in names])
+    hi = np.array([rows[n + "_hi"] for n in names])
+    t_mid = np.array([350.0, 300.0, 1000.0])       # junctions found in Table 1 (DESIGN.md reading T3)
+    net = SimpleNet([[2, 1], [2, 2], [1, 0]], lo, hi, t_mid, [BI], [[0, 0]], [[1, 2, 2]], [1],
+                    [[1e-11, 0.5, 1000.0]], element_names=["P", "O"])
+    T = np.array([280.0, 400.0, 900.0, 1500.0, 2500.0])
+    kf, kr = oracle.rate_coeffs(net, T, np.full(T.size, 1e6), None)
+
+    def g_rt(a, t):                                  # PAPER.md:671, exact rational arithmetic except ln T
+        a = [Fraction(float(x)) for x in a]
+        t = Fraction(float(t))
+        poly = -a[1] * t / 2 - a[2] * t ** 2 / 6 - a[3] * t ** 3 / 12 - a[4] * t ** 4 / 20 + a[5] / t - a[6]
+        return float(poly) + float(a[0]) * (1.0 - np.log(float(t)))
+
+    for c, t in enumerate(T):
+        sets = [lo[i] if t <= t_mid[i] else hi[i] for i in range(3)]
+        dg = g_rt(sets[1], t) + 2 * g_rt(sets[2], t) - 2 * g_rt(sets[0], t)
+        kc = np.exp(-dg) * P0 / (K_B * t)
+        assert kf[0, c] / kr[0, c] == pytest.approx(kc, rel=5e-12)
+        assert kf[0, c] == pytest.approx(1e-11 * t ** 0.5 * np.exp(-1000.0 / t), rel=1e-14)
