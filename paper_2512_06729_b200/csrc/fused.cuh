@@ -52,6 +52,7 @@ struct FusedArgs {
 
 __device__ __forceinline__ double2 lds2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
 __device__ __forceinline__ double2 ldg2(const unsigned char *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
+#ifndef XOD_EMU
 __device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
 }
@@ -59,6 +60,11 @@ __device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
+#else  // tests/kernel_emu: the kernel text compiled as host C++ (a copy completes at once)
+inline void cp_async16(void *smem, const void *gmem) { std::memcpy(smem, gmem, 16); }
+inline void cp_async8(void *smem, const void *gmem) { std::memcpy(smem, gmem, 8); }
+inline void cp_async_wait_all() {}
+#endif
 
 // log2 k_r (UNI/BI) or z (FALLOFF) from the block of interval g
 __device__ __forceinline__ double rev_eval(const unsigned char *blk, int slot16, double c0r /*C0*/, double T,

@@ -1,0 +1,113 @@
+"""The CUDA kernel SOURCE executed on CPU threads (tests/kernel_emu: one std::thread per CUDA thread,
+std::barrier as __syncthreads, blocks one after another) against the oracle.  No GPU needed: this
+checks the kernels' indexing, table decoding, chunk schedule and arithmetic as written, for the fused
+source kernel (both modes), its reaction-split/combine path, the persistent tile loop and the
+rate-coefficient kernel.  It cannot see races or memory-model effects; the `-m gpu` tests do that."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+from conftest import ROOT
+
+from paper_2512_06729_b200 import binding
+
+EMU_DIR = os.path.join(ROOT, "tests", "kernel_emu")
+CSRC = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
+LIB = os.path.join(EMU_DIR, "libxod_emu.so")
+SOURCES = [os.path.join(EMU_DIR, "emu.cpp"), os.path.join(CSRC, "pack.cpp"), os.path.join(CSRC, "pack_fused.cpp")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "xod_math.cuh", "xod_internal.h")] + [
+    os.path.join(EMU_DIR, "shim", "cuda_runtime.h")]
+
+
+@pytest.fixture(scope="module")
+def emu():
+    if not os.path.exists(LIB) or any(os.path.getmtime(d) > os.path.getmtime(LIB) for d in DEPS):
+        subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-shared", "-fPIC", "-DXOD_EMU",
+                        "-I" + os.path.join(EMU_DIR, "shim"), "-o", LIB] + SOURCES, check=True)
+    return C.CDLL(LIB)
+
+
+def descriptor(net):
+    keep = dict(
+        composition=np.ascontiguousarray(net.composition, dtype=np.int32), nasa_lo=np.ascontiguousarray(net.nasa_lo),
+        nasa_hi=np.ascontiguousarray(net.nasa_hi), t_mid=np.ascontiguousarray(net.t_mid),
+        type=np.ascontiguousarray(net.type, dtype=np.int32), reactants=np.ascontiguousarray(net.reactants, dtype=np.int32),
+        products=np.ascontiguousarray(net.products, dtype=np.int32), reversible=np.ascontiguousarray(net.reversible, dtype=np.uint8),
+        arrh=np.ascontiguousarray(net.arrh), arrh_low=np.ascontiguousarray(net.arrh_low),
+        troe_fc=np.ascontiguousarray(net.troe_fc), t_ref=np.ascontiguousarray(net.t_ref))
+    ns, ne = keep["composition"].shape
+    d = binding._Desc(ns, ne, keep["type"].shape[0], *[C.c_void_p(keep[k].ctypes.data) for k in (
+        "composition", "nasa_lo", "nasa_hi", "t_mid", "type", "reactants", "products", "reversible", "arrh",
+        "arrh_low", "troe_fc", "t_ref")], 0)
+    return d, keep
+
+
+def ptr(a):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def run_fused(emu, net, atm, ncol, kf=None, kr=None, grid=2, nsplit=1):
+    d, keep = descriptor(net)
+    out = np.full((net.n_species, atm.ld), np.nan)
+    rc = emu.emu_source_fused(C.byref(d), C.c_int64(ncol), C.c_int64(atm.ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                              ptr(kf), ptr(kr), ptr(atm.n), ptr(out), C.c_int(grid), C.c_int(nsplit))
+    assert rc == 0
+    return out
+
+
+def check(got, want, scale, ncol, what):
+    err = np.abs(got[:, :ncol] - want[:, :ncol])
+    assert np.all(err <= 1e-11 * scale[:, :ncol]), what
+    assert np.all(np.isnan(got[:, ncol:])), what + ": padding columns written"
+
+
+@pytest.mark.parametrize("cfg,grid,nsplit", [(1, 1, 1), (1, 2, 1), (2, 3, 1), (2, 5, 3)])
+def test_fused_kernel_source_matches_oracle(emu, oracle, network, cfg, grid, nsplit):
+    """k_fused<false> (a1-a8): config 1 (one chunk, 2 tiles) and config 2 (3 chunks, 8 tiles) with fewer
+    blocks than work items (persistent loop) and with the chunks of a tile split over blocks."""
+    from paper_2512_06729_b200 import synth
+    net = network(cfg)
+    atm = synth.config_atmosphere(cfg, net)
+    want, wp, wl = oracle.source_from_state(net, atm.T, atm.P, atm.J, atm.n, atm.ncol)
+    got = run_fused(emu, net, atm, atm.ncol, grid=grid, nsplit=nsplit)
+    check(got, want, wp + wl, atm.ncol, "emulated k_fused config %d" % cfg)
+
+
+def test_fused_kernel_source_from_stored_coefficients_and_mixed_intervals(emu, oracle, network):
+    """k_fused<true> (xod_source), and a tile whose columns straddle thermo breakpoints (the rare
+    per-thread second parameter block) with cold columns whose k_r overflow."""
+    from paper_2512_06729_b200 import synth
+    net = network(2)
+    atm = synth.make_atmosphere(5, net, 1, 37, t_shift=(-600.0, -600.0))
+    atm.T[:37] = np.linspace(180.0, 1100.0, 37)          # crosses 300, 500, 700, 1000 K inside tiles
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    fin = np.all(np.isfinite(okr[:, :atm.ncol]), axis=0) & np.all(np.isfinite(want[:, :atm.ncol]), axis=0)
+    assert 5 < fin.sum() < atm.ncol
+    got = run_fused(emu, net, atm, atm.ncol, grid=2)
+    err = np.abs(got[:, :atm.ncol] - want[:, :atm.ncol])[:, fin]
+    assert np.all(err <= 1e-11 * (wp + wl)[:, :atm.ncol][:, fin])
+    got_k = run_fused(emu, net, atm, atm.ncol, kf=np.ascontiguousarray(okf), kr=np.ascontiguousarray(okr), grid=3)
+    err = np.abs(got_k[:, :atm.ncol] - want[:, :atm.ncol])[:, fin]
+    assert np.all(err <= 1e-11 * (wp + wl)[:, :atm.ncol][:, fin])
+
+
+@pytest.mark.parametrize("cfg,slice_", [(1, 64), (2, 8)])
+def test_rate_coefficient_kernel_source_matches_oracle(emu, oracle, network, cfg, slice_):
+    from paper_2512_06729_b200 import synth
+    net = network(cfg)
+    atm = synth.config_atmosphere(cfg, net)
+    d, keep = descriptor(net)
+    kf = np.full((net.n_reactions, atm.ld), np.nan)
+    kr = np.full((net.n_reactions, atm.ld), np.nan)
+    rc = emu.emu_rate_coeffs(C.byref(d), C.c_int64(atm.ncol), C.c_int64(atm.ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                             ptr(kf), ptr(kr), C.c_int(slice_))
+    assert rc == 0
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    c = slice(0, atm.ncol)
+    assert np.all(np.abs(kf[:, c] - okf[:, c]) <= 1e-12 * np.abs(okf[:, c]))
+    assert np.all(np.abs(kr[:, c] - okr[:, c]) <= 1e-12 * np.abs(okr[:, c]))
+    assert np.all(np.isnan(kf[:, atm.ncol:])) and np.all(np.isnan(kr[:, atm.ncol:]))
