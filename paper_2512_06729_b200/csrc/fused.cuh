@@ -85,7 +85,11 @@ __device__ __forceinline__ size_t block_offset(const FusedDev &f, int pp) {
 
 template <bool FROMK>
 __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, FusedArgs a) {
+#ifndef XOD_EMU
   extern __shared__ __align__(16) unsigned char smem_raw[];
+#else
+  extern unsigned char smem_raw[];  // tests/kernel_emu provides the CTA's shared memory
+#endif
   double *n_s = reinterpret_cast<double *>(smem_raw);
   double *acc_s = n_s + (size_t)(ns + 1) * kFW;
   double *q_s = acc_s + (size_t)f.n_acc * kFW;

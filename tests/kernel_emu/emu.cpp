@@ -17,6 +17,7 @@ void emu_syncthreads() { g_barrier->arrive_and_wait(); }
 
 #include "../../paper_2512_06729_b200/csrc/fused.cuh"
 #include "../../paper_2512_06729_b200/csrc/rates2.cuh"
+#include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
 alignas(16) unsigned char smem_raw[256 * 1024];  // the CTA's dynamic shared memory
@@ -117,6 +118,99 @@ int emu_rate_coeffs(const xod_network_desc *d, int64_t ncol, int64_t ld, const d
   if (!pack(d, h, fd) || ncol <= 0) return 1;
   run_grid((unsigned)((ncol + 255) / 256), (unsigned)((fd.ph_end + slice - 1) / slice), 256, false,
            [&] { k_rate_coeffs(fd, ncol, ld, T, P, J, kf, kr, kLog2Kb, slice); });
+  return 0;
+}
+
+// ---- the multi-kernel entry points (kernels.cuh): thermo, Jacobian, and the prologue -> rates -> source
+// pipeline that serves the prod/loss variants and the fallback of the fused path
+static DevTables dev_tables(const HostTables &h) {
+  DevTables d{};
+  d.ns = h.ns, d.nr = h.nr, d.n_photo = h.n_photo;
+  d.uni_begin = h.uni_begin, d.bi_begin = h.bi_begin, d.fo_begin = h.fo_begin, d.ph_begin = h.ph_begin;
+  d.c0 = h.c0.data(), d.c1 = h.c1.data(), d.c2 = h.c2.data();
+  d.l0 = h.l0.data(), d.l1 = h.l1.data(), d.l2 = h.l2.data(), d.fcl = h.fcl.data(), d.cN = h.cN.data();
+  d.sp = h.sp.data(), d.flags = h.flags.data(), d.user = h.packed_to_user.data(), d.photo_row = h.photo_row.data();
+  d.nasa = h.nasa.data(), d.nasa_l2 = h.nasa_l2.data(), d.tmid = h.tmid.data();
+  d.src_rxn = h.src_rxn_packed.data(), d.src_nu = h.src_nu_f.data(), d.src_seg = h.src_seg.data();
+  d.n_src_tasks = (int32_t)(h.src_seg.size() / kSrcWarpsPerCta);
+  d.jac_term_ptr = h.jac_term_ptr.data(), d.jac_terms = h.jac_terms.data();
+  d.nnz_jac = (int64_t)h.jac_col.size();
+  return d;
+}
+
+int emu_thermo(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *T, double *cp, double *hh,
+               double *ss, double *gg, int spb) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK) return 1;
+  const DevTables d = dev_tables(h);
+  run_grid((unsigned)((ncol + 127) / 128), (unsigned)((h.ns + spb - 1) / spb), 128, false,
+           [&] { k_thermo(d, ncol, ld, T, cp, hh, ss, gg, spb); });
+  return 0;
+}
+
+int emu_jacobian(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                 const double *n, double *jac, int gx) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK) return 1;
+  const DevTables d = dev_tables(h);
+  run_grid((unsigned)gx, (unsigned)((ncol + 31) / 32), 256, false, [&] { k_jacobian(d, ncol, ld, kf, kr, n, jac); });
+  return 0;
+}
+
+// (T, P, J, n) -> dn/dt [, P, L] through k_prologue + k_rates + k_source; with kf_in/kr_in given, through
+// k_rates_from_k + k_source instead (xod_source with prod/loss).  One chunk holds all columns.
+int emu_source_pipeline(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *T, const double *P,
+                        const double *J, const double *kf_in, const double *kr_in, const double *n, double *dndt,
+                        double *prod, double *loss, int rw) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK) return 1;
+  const DevTables d = dev_tables(h);
+  const int64_t ldw = (ncol + 31) / 32 * 32, ncg = ldw / 32;
+  const bool pl = prod != nullptr;
+  std::vector<double> buf((size_t)(3 + h.ns + 2 * (size_t)h.nr) * ldw);
+  ChunkScratch w{};
+  w.ldw = ldw;
+  w.l2T = buf.data(), w.invT = w.l2T + ldw, w.lM = w.invT + ldw, w.u = w.lM + ldw;
+  w.q = w.u + (size_t)h.ns * ldw, w.qr = w.q + (size_t)h.nr * ldw;
+  const int64_t nslices = (h.nr + rw - 1) / rw, ntasks = nslices * ncg;
+  const unsigned blocks = (unsigned)((ntasks + 3) / 4);
+  if (!kf_in) {
+    run_grid((unsigned)ncg, 2, 256, false, [&] { k_prologue(d, ncol, 0, T, P, w, kLog2Kb); });
+    if (pl)
+      run_grid(blocks, 1, 128, false, [&] { k_rates<MODE_QSEP>(d, ncol, 0, ld, w, J, n, nullptr, nullptr, rw, (int)ncg, ntasks); });
+    else
+      run_grid(blocks, 1, 128, false, [&] { k_rates<MODE_QNET>(d, ncol, 0, ld, w, J, n, nullptr, nullptr, rw, (int)ncg, ntasks); });
+  } else if (pl) {
+    run_grid(blocks, 1, 128, false, [&] { k_rates_from_k<MODE_QSEP>(d, ncol, 0, ld, w, kf_in, kr_in, n, rw, (int)ncg, ntasks); });
+  } else {
+    run_grid(blocks, 1, 128, false, [&] { k_rates_from_k<MODE_QNET>(d, ncol, 0, ld, w, kf_in, kr_in, n, rw, (int)ncg, ntasks); });
+  }
+  if (pl)
+    run_grid((unsigned)d.n_src_tasks, (unsigned)ncg, 256, true, [&] { k_source<true>(d, ncol, 0, ld, w, dndt, prod, loss); });
+  else
+    run_grid((unsigned)d.n_src_tasks, (unsigned)ncg, 256, true, [&] { k_source<false>(d, ncol, 0, ld, w, dndt, prod, loss); });
+  return 0;
+}
+
+// k_f, k_r in USER order through k_prologue + k_rates<MODE_K> (the fallback of xod_rate_coeffs)
+int emu_rate_coeffs_pipeline(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *T, const double *P,
+                             const double *J, double *kf, double *kr, int rw) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK) return 1;
+  const DevTables d = dev_tables(h);
+  const int64_t ldw = (ncol + 31) / 32 * 32, ncg = ldw / 32;
+  std::vector<double> buf((size_t)(3 + h.ns) * ldw);
+  ChunkScratch w{};
+  w.ldw = ldw;
+  w.l2T = buf.data(), w.invT = w.l2T + ldw, w.lM = w.invT + ldw, w.u = w.lM + ldw;
+  const int64_t ntasks = (int64_t)((h.nr + rw - 1) / rw) * ncg;
+  run_grid((unsigned)ncg, 1, 256, false, [&] { k_prologue(d, ncol, 0, T, P, w, kLog2Kb); });
+  run_grid((unsigned)((ntasks + 3) / 4), 1, 128, false,
+           [&] { k_rates<MODE_K>(d, ncol, 0, ld, w, J, nullptr, kf, kr, rw, (int)ncg, ntasks); });
   return 0;
 }
 

@@ -14,7 +14,7 @@
 #define __forceinline__ inline
 #define __noinline__
 #define __constant__
-#define __shared__
+#define __shared__ static   /* blocks run one after another, so one copy per kernel is the CTA's */
 #define __launch_bounds__(...)
 #define __align__(n) __attribute__((aligned(n)))
 
@@ -52,4 +52,4 @@ inline long min(long a, long b) { return a < b ? a : b; }
 inline long max(long a, long b) { return a > b ? a : b; }
 inline long long min(long long a, long long b) { return a < b ? a : b; }
 inline long long max(long long a, long long b) { return a > b ? a : b; }
-using std::fabs; using std::fma; using std::fmax; using std::fmin; using std::log2;
+using std::fabs; using std::fma; using std::fmax; using std::fmin; using std::log; using std::log2;

@@ -18,7 +18,7 @@ EMU_DIR = os.path.join(ROOT, "tests", "kernel_emu")
 CSRC = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
 LIB = os.path.join(EMU_DIR, "libxod_emu.so")
 SOURCES = [os.path.join(EMU_DIR, "emu.cpp"), os.path.join(CSRC, "pack.cpp"), os.path.join(CSRC, "pack_fused.cpp")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "xod_math.cuh", "xod_internal.h")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "xod_math.cuh", "xod_internal.h")] + [
     os.path.join(EMU_DIR, "shim", "cuda_runtime.h")]
 
 
@@ -111,3 +111,57 @@ def test_rate_coefficient_kernel_source_matches_oracle(emu, oracle, network, cfg
     assert np.all(np.abs(kf[:, c] - okf[:, c]) <= 1e-12 * np.abs(okf[:, c]))
     assert np.all(np.abs(kr[:, c] - okr[:, c]) <= 1e-12 * np.abs(okr[:, c]))
     assert np.all(np.isnan(kf[:, atm.ncol:])) and np.all(np.isnan(kr[:, atm.ncol:]))
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_thermo_and_jacobian_kernel_sources_match_oracle(emu, oracle, network, cfg):
+    from paper_2512_06729_b200 import synth
+    net = network(cfg)
+    atm = synth.config_atmosphere(cfg, net)
+    d, keep = descriptor(net)
+    ns, ld, ncol = net.n_species, atm.ld, atm.ncol
+    outs = [np.full((ns, ld), np.nan) for _ in range(4)]
+    assert emu.emu_thermo(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), *[ptr(o) for o in outs], C.c_int(5)) == 0
+    want = oracle.thermo(net, atm.T, ncol)
+    for got, w in zip(outs, want):
+        assert np.all(np.abs(got[:, :ncol] - w[:, :ncol]) <= 1e-12 * (1 + np.abs(w[:, :ncol])))
+        assert np.all(np.isnan(got[:, ncol:]))
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    h = binding.Network(net, device=-1)
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
+    jac = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr), ptr(atm.n), ptr(jac), C.c_int(3)) == 0
+    assert np.all(np.abs(jac[:, :ncol] - wj[:, :ncol]) <= 1e-11 * sj[:, :ncol])
+    assert np.all(np.isnan(jac[:, ncol:]))
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_multi_kernel_pipeline_sources_match_oracle(emu, oracle, network, cfg):
+    """k_prologue + k_rates + k_source (the prod/loss variants and the fallback of the fused path), and
+    k_rates_from_k + k_source for xod_source with prod/loss."""
+    from paper_2512_06729_b200 import synth
+    net = network(cfg)
+    atm = synth.config_atmosphere(cfg, net)
+    d, keep = descriptor(net)
+    ns, ld, ncol = net.n_species, atm.ld, atm.ncol
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    scale = wp + wl
+    for kf_in, kr_in in ((None, None), (okf, okr)):
+        for pl in (False, True):
+            dn, pr, lo = (np.full((ns, ld), np.nan) for _ in range(3))
+            rc = emu.emu_source_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                                         ptr(kf_in), ptr(kr_in), ptr(atm.n), ptr(dn), ptr(pr) if pl else None,
+                                         ptr(lo) if pl else None, C.c_int(16))
+            assert rc == 0
+            check(dn, want, scale, ncol, "pipeline dn/dt")
+            if pl:
+                check(pr, wp, scale, ncol, "pipeline P")
+                check(lo, wl, scale, ncol, "pipeline L")
+    kf = np.full((net.n_reactions, ld), np.nan)
+    kr = np.full((net.n_reactions, ld), np.nan)
+    assert emu.emu_rate_coeffs_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                                        ptr(kf), ptr(kr), C.c_int(16)) == 0
+    assert np.all(np.abs(kf[:, :ncol] - okf[:, :ncol]) <= 1e-12 * np.abs(okf[:, :ncol]))
+    assert np.all(np.abs(kr[:, :ncol] - okr[:, :ncol]) <= 1e-12 * np.abs(okr[:, :ncol]))
