@@ -44,7 +44,7 @@ NOMINAL_DFMA_PER_S = 148 * 64 * 1.965e9   # 148 SMs x 64 FP64 lanes x clocks.max
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)   # 0.26 s timed region: several clock samples
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4", choices=["config3", "config4", "config5"])
