@@ -165,3 +165,38 @@ def test_multi_kernel_pipeline_sources_match_oracle(emu, oracle, network, cfg):
                                         ptr(kf), ptr(kr), C.c_int(16)) == 0
     assert np.all(np.abs(kf[:, :ncol] - okf[:, :ncol]) <= 1e-12 * np.abs(okf[:, :ncol]))
     assert np.all(np.abs(kr[:, :ncol] - okr[:, :ncol]) <= 1e-12 * np.abs(okr[:, :ncol]))
+
+
+TSAN_CHILD = r"""
+import sys, ctypes as C
+sys.path.insert(0, sys.argv[1]); sys.path.insert(0, sys.argv[1] + "/tests")
+import numpy as np
+import test_kernel_emulation as tk
+from paper_2512_06729_b200 import synth
+emu = C.CDLL(sys.argv[2])
+net = synth.config_network(2)
+atm = synth.config_atmosphere(2, net)
+for grid, nsplit in ((3, 1), (5, 3)):
+    got = tk.run_fused(emu, net, atm, atm.ncol, grid=grid, nsplit=nsplit)
+    assert np.all(np.isfinite(got[:, :atm.ncol]))
+print("emulated-ok")
+"""
+
+
+def test_fused_kernel_source_is_race_free_under_thread_sanitizer():
+    """racecheck substitute (compute-sanitizer is closed on the GPU pool): the emulated CUDA threads are
+    real threads and __syncthreads a real barrier, so ThreadSanitizer sees every shared-memory access
+    of k_fused between barriers: the double-buffered q and schedule, the accumulator read-modify-writes
+    of the row tasks, the tile prologue/epilogue.  (Removing the per-chunk barrier makes it report.)"""
+    tsan = subprocess.run(["gcc", "-print-file-name=libtsan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(tsan) or not os.path.exists(tsan):
+        pytest.skip("libtsan not available")
+    lib = os.path.join(EMU_DIR, "libxod_emu_tsan.so")
+    if not os.path.exists(lib) or any(os.path.getmtime(d) > os.path.getmtime(lib) for d in DEPS):
+        subprocess.run(["g++", "-std=c++20", "-O1", "-g", "-fsanitize=thread", "-pthread", "-shared", "-fPIC", "-DXOD_EMU",
+                        "-I" + os.path.join(EMU_DIR, "shim"), "-o", lib] + SOURCES, check=True)
+    env = dict(os.environ, LD_PRELOAD=tsan, TSAN_OPTIONS="halt_on_error=0 report_signal_unsafe=0 exitcode=0")
+    out = subprocess.run([os.sys.executable, "-c", TSAN_CHILD, ROOT, lib], capture_output=True, text=True, env=env,
+                         timeout=900)
+    assert "emulated-ok" in out.stdout, out.stderr[-2000:]
+    assert "ThreadSanitizer" not in out.stderr, out.stderr[-3000:]
