@@ -141,21 +141,32 @@ xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launch
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);
 
-/* ---- a2: NASA-7 thermochemistry.  T [ld]; each output [n_species][ld], any may be NULL. */
+/* ---- a2: NASA-7 thermochemistry (PAPER.md:650-653 two coefficient sets; PAPER.md:671 G/RT, 673 cp/R;
+ * H/RT, S/R standard forms, reading T1; set chosen by T <= t_mid, reading T3).  T [ld] device;
+ * each output [n_species][ld] device, any may be NULL; columns >= ncol are not touched.
+ * Errors: XOD_ERR_INVALID_ARG (NULL T, ncol < 0, ld < ncol), XOD_ERR_CUDA. */
 xod_status xod_thermo(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
                       double *cp_R, double *h_RT, double *s_R, double *g_RT, void *stream);
 
-/* ---- a1, a3-a6: forward and reverse rate coefficients.  T, P [ld]; J [n_photo][ld] (may be NULL
- * if n_photo == 0); kf, kr [n_reactions][ld] in user order, either may be NULL.  kr rows of
- * irreversible and photolysis reactions are 0. */
+/* ---- a1, a3-a6: forward and reverse rate coefficients: Eq. 7, Eq. 10-12 with
+ * [M] = P/(k_B T) and Troe F (reading F1), k_f = J for photolysis,
+ * k_r = k_f/K_c, K_c = exp(-dG/RT)(P0/k_B T)^dnu (Eq. 13-15).  T, P [ld]; J
+ * [n_photo][ld] (may be NULL if n_photo == 0); kf, kr [n_reactions][ld] in user order, either may be
+ * NULL; all device memory owned by the caller.  kr rows of irreversible and photolysis reactions are
+ * 0; values beyond the double range saturate as IEEE does (reading R5).  The workspace (device,
+ * >= xod_rate_coeffs_workspace_bytes) is only used by the multi-kernel fallback.
+ * Errors: XOD_ERR_INVALID_ARG, XOD_ERR_WORKSPACE, XOD_ERR_CUDA; nothing is enqueued on error. */
 size_t xod_rate_coeffs_workspace_bytes(const xod_network *net, int64_t ncol);
 xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
                            const double *P, const double *J, double *kf, double *kr,
                            void *workspace, size_t workspace_bytes, void *stream);
 
-/* ---- a7-a8: dn/dt from stored coefficients.  n [n_species][ld]; dndt [n_species][ld];
- * prod, loss optional (both or neither): P_i = sum of positive terms, L_i = sum of |negative
- * terms|, dn/dt = P - L. */
+/* ---- a7-a8: dn/dt from stored coefficients: q_f = k_f prod n_reactant, q_r = k_r prod n_product
+ * (north_star; PAPER.md:211 for photolysis), dn_i/dt = P_i - L_i = sum_r nu_ir (q_f,r - q_r,r)
+ * (Eq. 1).  kf, kr [n_reactions][ld] user order; n, dndt [n_species][ld]; prod, loss
+ * optional (both or neither): P_i = sum of positive terms, L_i = sum of |negative terms|.  Device
+ * memory owned by the caller; workspace >= xod_source_workspace_bytes(net, ncol).
+ * Errors: XOD_ERR_INVALID_ARG, XOD_ERR_WORKSPACE, XOD_ERR_CUDA. */
 size_t xod_source_workspace_bytes(const xod_network *net, int64_t ncol);
 xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
                       const double *kr, const double *n, double *dndt, double *prod, double *loss,
@@ -168,7 +179,11 @@ xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, co
                             double *prod, double *loss, void *workspace, size_t workspace_bytes,
                             void *stream);
 
-/* ---- a9: Jacobian values jac[e][col], e over the pattern of xod_network_jac_pattern. */
+/* ---- a9: Jacobian values jac[e][col] = d(dn_i/dt)/dn_j for entry e = (i, j) of the pattern of
+ * xod_network_jac_pattern (BASELINE.json config 5; k_f, k_r, [M], J do not depend on n, reading J3):
+ * sum_r nu_ir (d q_f,r/d n_j - d q_r,r/d n_j), never formed as q/n_j, so n_j = 0 is exact (reading Q2).
+ * kf, kr [n_reactions][ld], n [n_species][ld], jac [nnz_jac][ld]: device memory owned by the caller.
+ * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, ncol > 2097120), XOD_ERR_CUDA. */
 xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
                         const double *kr, const double *n, double *jac, void *stream);
 
