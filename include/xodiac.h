@@ -22,8 +22,11 @@
  *               reaction in user order.  The type-sorted order is internal (xod_network_perm).
  *   Memory      xod_network_desc pointers are HOST memory, copied by create.  Every pointer of a
  *               compute call is DEVICE memory owned by the caller, except in the *_host call.
- *   Streams     `stream` is a cudaStream_t passed as void* (NULL = default stream).  Compute
- *               calls only enqueue work and never synchronise; the *_host call synchronises.
+ *   Streams     `stream` is a cudaStream_t passed as void* (NULL = default stream) of the network's
+ *               device, which must be the calling thread's current device (otherwise XOD_ERR_CUDA;
+ *               the library never switches the caller's device).  Compute calls only enqueue work,
+ *               never synchronise and may be captured into a CUDA graph; the *_host call
+ *               synchronises.
  *   Errors      argument problems return synchronously with nothing enqueued; xod_last_error()
  *               (thread-local) says what was wrong.  IEEE overflow/underflow in results (k_r
  *               beyond the double range, reading R5) is not an error.
@@ -194,6 +197,15 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
  * streams are owned by the network and grown on demand (not thread-safe on one network). */
 xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, const double *T,
                                  const double *P, const double *J, const double *n, double *dndt);
+
+/* ---- debugging: synchronises the network's device and returns XOD_OK, or XOD_ERR_CUDA if the
+ * device reports an error.  In the bounds-checked build of the library (-DXOD_CHECK, built by
+ * `XOD_CHECK=1 python -m paper_2512_06729_b200.build`; xod_build_has_checks() == 1) every index a
+ * kernel derives from the packed tables is range-checked and clamped, and this call reports the
+ * first violation (kernel source line in xod_last_error) instead of the GPU faulting.  The default
+ * build has no such code in its kernels. */
+xod_status xod_check_status(const xod_network *net);
+int32_t xod_build_has_checks(void);
 
 /* ---- measurement helper: sustained DFMA issue rate of the device (dependent-chain-free FMA
  * loop on every SM), used as the FP64 roofline denominator.  Returns fused multiply-adds per

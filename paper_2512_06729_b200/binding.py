@@ -9,7 +9,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libxodiac.so")
+# XOD_CHECK=1 selects the bounds-checked debugging build (same sources, -DXOD_CHECK; see build.py)
+_LIB_PATH = os.path.join(_HERE, "libxodiac_check.so" if os.environ.get("XOD_CHECK") else "libxodiac.so")
 _lib = None
 
 XOD_OK = 0
@@ -25,7 +26,8 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_network_jac_pattern", "xod_network_tune", "xod_thermo",
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
-           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params"]
+           "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params",
+           "xod_check_status", "xod_build_has_checks"]
 
 
 class XodError(RuntimeError):
@@ -48,7 +50,7 @@ def lib():
     global _lib
     if _lib is None:
         if not os.path.exists(_LIB_PATH):
-            raise RuntimeError("libxodiac.so is missing: run `python -m paper_2512_06729_b200.build` "
+            raise RuntimeError(os.path.basename(_LIB_PATH) + " is missing: run `python -m paper_2512_06729_b200.build` "
                                "(there is no CPU fallback)")
         L = C.CDLL(_LIB_PATH)
         L.xod_last_error.restype = C.c_char_p
@@ -166,6 +168,10 @@ class Network:
     def selfcheck(self):
         _check(lib().xod_network_selfcheck(self._h))
 
+    def check_status(self):
+        """Synchronise the device; in the XOD_CHECK build raise if a kernel saw an out-of-range table index."""
+        _check(lib().xod_check_status(self._h))
+
     def tune(self, knob, value):
         _check(lib().xod_network_tune(self._h, C.c_int32(knob), C.c_int64(value)))
 
@@ -225,6 +231,10 @@ class Network:
             return C.c_void_p(a.data_ptr())
         _check(lib().xod_source_fused_host(self._h, C.c_int64(ncol), C.c_int64(ld), hp(T), hp(P), hp(J),
                                            hp(n), hp(dndt)))
+
+
+def build_has_checks():
+    return bool(lib().xod_build_has_checks())
 
 
 def launch_count():

@@ -7,9 +7,10 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "libxodiac.so")
+CHECKED = bool(os.environ.get("XOD_CHECK"))   # debugging build: bounds-checked table indices (csrc/xod_cta.cuh)
+LIB = os.path.join(HERE, "libxodiac_check.so" if CHECKED else "libxodiac.so")
 SOURCES = ["api.cu", "pack.cpp", "pack_fused.cpp"]
-HEADERS = ["kernels.cuh", "fused.cuh", "rates2.cuh", "xod_math.cuh", "xod_internal.h", os.path.join("..", "..", "include", "xodiac.h")]
+HEADERS = ["kernels.cuh", "fused.cuh", "rates2.cuh", "xod_math.cuh", "xod_cta.cuh", "xod_internal.h", os.path.join("..", "..", "include", "xodiac.h")]
 
 
 def _stale():
@@ -24,11 +25,11 @@ def build(force=False, verbose=False):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-           "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", LIB]
+           "-I" + CSRC, "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    if os.environ.get("XOD_ABLATE"):      # profiling builds only: phase ablation switches in k_fused
-        cmd += ["-DXOD_ABLATE"]
+    if CHECKED:
+        cmd += ["-DXOD_CHECK"]
     cmd += [os.path.join(CSRC, f) for f in SOURCES]
     subprocess.run(cmd, check=True)
     return LIB

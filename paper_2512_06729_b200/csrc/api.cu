@@ -106,6 +106,10 @@ ChunkScratch carve(const xod_network *net, void *ws, int64_t ldw, bool need_u, b
   return s;
 }
 
+// Argument checks common to the compute calls.  The compute calls only enqueue kernels on the
+// caller's stream; they never change the calling thread's current device (a mismatch is an error,
+// not a silent switch: include/xodiac.h, "Streams") and they are legal inside a CUDA graph capture
+// (cudaGetDevice is a thread-local read, not a stream operation).
 xod_status check_common(const xod_network *net, int64_t ncol, int64_t ld) {
   if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
   if (ncol < 0) return fail(XOD_ERR_INVALID_ARG, "ncol < 0");
@@ -113,13 +117,28 @@ xod_status check_common(const xod_network *net, int64_t ncol, int64_t ld) {
   if (net->device < 0) return fail(XOD_ERR_CUDA, "network was created without a CUDA device");
   int cur = -1;
   XOD_CUDA(cudaGetDevice(&cur));
-  if (cur != net->device) XOD_CUDA(cudaSetDevice(net->device));
+  if (cur != net->device) return fail(XOD_ERR_CUDA, "the calling thread's current CUDA device is not the network's device");
   return XOD_OK;
 }
 
+// Makes `device` current for the lifetime of the guard and restores the caller's device on every
+// exit path (create, the *_host call and the probe allocate or synchronise, so they need it).
+struct DeviceGuard {
+  int prev = -1;
+  cudaError_t err = cudaSuccess;
+  explicit DeviceGuard(int device) {
+    err = cudaGetDevice(&prev);
+    if (err == cudaSuccess && prev != device) err = cudaSetDevice(device);
+  }
+  ~DeviceGuard() {
+    int cur = -1;
+    if (prev >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev) cudaSetDevice(prev);
+  }
+};
+
 // reactions per warp task: aim at ~2 resident waves of warps over the whole chip
-int pick_rw(int nr, int64_t ncg) {
-  const int64_t target = 148LL * 32 * 2;
+int pick_rw(const xod_network *net, int nr, int64_t ncg) {
+  const int64_t target = (int64_t)net->sm_count * 32 * 2;
   int64_t rw = ((int64_t)nr * ncg + target - 1) / target;
   return (int)std::min<int64_t>(std::max<int64_t>(rw, 8), 128);
 }
@@ -160,12 +179,10 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
     return fail(XOD_ERR_ALLOC, "out of host memory while packing");
   }
   if (cuda_device >= 0) {
-    int prev = -1;
-    cudaError_t e = cudaGetDevice(&prev);
-    if (e == cudaSuccess) e = cudaSetDevice(cuda_device);
-    if (e != cudaSuccess) {
+    DeviceGuard guard(cuda_device);
+    if (guard.err != cudaSuccess) {
       delete net;
-      return cuda_fail(e, "cudaSetDevice");
+      return cuda_fail(guard.err, "cudaSetDevice");
     }
     HostTables &h = net->h;
     DevTables &d = net->d;
@@ -211,7 +228,6 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
         net->sm_count = smc;
     }
 #undef UP
-    if (prev >= 0 && prev != cuda_device) cudaSetDevice(prev);
     if (st != XOD_OK) {
       std::string keep = g_err;
       xod_network_destroy(net);
@@ -325,10 +341,6 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
     net->chunk_cols = value;
     return XOD_OK;
   }
-  if (knob == 99) {  // undocumented: ablation switches of k_fused (profiling only)
-    net->debug = value;
-    return XOD_OK;
-  }
   if (knob == XOD_TUNE_SPLIT) {
     if (value < 0) return fail(XOD_ERR_INVALID_ARG, "split must be >= 0");
     net->force_split = value;
@@ -358,7 +370,7 @@ xod_status xod_thermo(const xod_network *net, int64_t ncol, int64_t ld, const do
   const int64_t gx = (ncol + 127) / 128;
   // enough CTAs to fill the chip even for one atmosphere: split the species over blockIdx.y
   int spb = net->h.ns;
-  while (spb > 4 && gx * ((net->h.ns + spb - 1) / spb) < 148 * 8) spb = (spb + 1) / 2;
+  while (spb > 4 && gx * ((net->h.ns + spb - 1) / spb) < (int64_t)net->sm_count * 8) spb = (spb + 1) / 2;
   dim3 grid((unsigned)gx, (unsigned)((net->h.ns + spb - 1) / spb));
   {
     Timed tm(net, KID_THERMO, s);
@@ -380,7 +392,7 @@ namespace {
 xod_status launch_prologue(const xod_network *net, int64_t ncol, int64_t col0, int64_t ncg,
                            const double *T, const double *P, const ChunkScratch &w, cudaStream_t s) {
   int split = 1;
-  while (split < 64 && ncg * split < 148 * 2 && split * 8 < net->h.ns) split *= 2;
+  while (split < 64 && ncg * split < (int64_t)net->sm_count * 2 && split * 8 < net->h.ns) split *= 2;
   dim3 grid((unsigned)ncg, (unsigned)split);
   {
     Timed tm(net, KID_PROLOGUE, s);
@@ -394,10 +406,10 @@ template <int MODE>
 xod_status launch_rates(const xod_network *net, int64_t ncol, int64_t col0, int64_t ld, int64_t ncg,
                         const ChunkScratch &w, const double *J, const double *n, double *kf, double *kr,
                         cudaStream_t s) {
-  const int rw = pick_rw(net->h.nr, ncg);
+  const int rw = pick_rw(net, net->h.nr, ncg);
   const int64_t nslices = (net->h.nr + rw - 1) / rw;
   const int64_t ntasks = nslices * ncg;
-  const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, 148LL * 16);
+  const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, (int64_t)net->sm_count * 16);
   {
     Timed tm(net, KID_RATES, s);
     k_rates<MODE><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, J, n, kf, kr, rw, (int)ncg, ntasks);
@@ -446,7 +458,7 @@ xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const 
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
   a.nsplit = fused_split(net, ncol);
   a.log2_kb = kLog2Kb;
-  a.debug = (int32_t)net->debug;
+  a.nr = h.nr, a.n_photo = h.n_photo;
   a.ldp = round_up(ncol, 32);
   double *part = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
   a.out = a.nsplit == 1 ? dndt : part;
@@ -505,7 +517,7 @@ xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, con
     slice = (slice + 3) / 4 * 4;
     dim3 grid((unsigned)nbx, (unsigned)((net->fd.ph_end + slice - 1) / slice));
     Timed tm(net, KID_RATE_COEFFS, s);
-    k_rate_coeffs<<<grid, 256, 0, s>>>(net->fd, ncol, ld, T, P, J, kf, kr, kLog2Kb, slice);
+    k_rate_coeffs<<<grid, 256, 0, s>>>(net->fd, ncol, ld, T, P, J, kf, kr, kLog2Kb, slice, net->h.nr, net->h.n_photo);
     XOD_CUDA(cudaGetLastError());
     return XOD_OK;
   }
@@ -544,9 +556,9 @@ xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const do
   for (int64_t col0 = 0; col0 < ncol; col0 += ldw) {
     const int64_t nc = std::min(ldw, ncol - col0), ncg = (nc + 31) / 32;
     if (net->h.nr > 0) {
-      const int rw = pick_rw(net->h.nr, ncg);
+      const int rw = pick_rw(net, net->h.nr, ncg);
       const int64_t ntasks = (int64_t)((net->h.nr + rw - 1) / rw) * ncg;
-      const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, 148LL * 16);
+      const int64_t blocks = std::min<int64_t>((ntasks + 3) / 4, (int64_t)net->sm_count * 16);
       Timed tm(net, KID_RATES_FROM_K, s);
       if (pl)
         k_rates_from_k<MODE_QSEP><<<(unsigned)blocks, 128, 0, s>>>(net->d, ncol, col0, ld, w, kf, kr, n, rw, (int)ncg, ntasks);
@@ -624,6 +636,10 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
 
 xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, const double *T,
                                  const double *P, const double *J, const double *n, double *dndt) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  if (net->device < 0) return fail(XOD_ERR_CUDA, "network was created without a CUDA device");
+  DeviceGuard guard(net->device);  // this call allocates and synchronises: it may switch, and restores
+  if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
   xod_status st = check_common(net, ncol, ld);
   if (st != XOD_OK) return st;
   if (ncol == 0) return XOD_OK;
@@ -635,7 +651,9 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
   // costs the persistent kernel no tail.  Rows are strided in host memory: cudaMemcpy2DAsync.
   const size_t ns = net->h.ns, nph = net->h.n_photo;
   const int64_t cw = std::min<int64_t>(round_up(ncol, 32), (int64_t)net->sm_count * kFW);  // columns per chunk
-  const size_t ws = xod_source_fused_workspace_bytes(net, cw) + 256;
+  // the ragged last chunk runs with fewer tiles and therefore more reaction splits: size for both widths
+  const size_t ws = std::max(xod_source_fused_workspace_bytes(net, cw),
+                             ncol % cw ? xod_source_fused_workspace_bytes(net, ncol % cw) : 0) + 256;
   const size_t rows = 2 + nph + 2 * ns;
   const size_t slot_bytes = round_up((int64_t)(rows * cw * sizeof(double) + ws), 256);
   const size_t need = slot_bytes * kHostSlots;
@@ -652,6 +670,19 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
       net->host_streams[i] = s;
     }
   const size_t hp = (size_t)ld * sizeof(double), dp = (size_t)cw * sizeof(double);
+  // an error after the first chunk must not return with copies still in flight on the private streams
+  auto drain = [&](xod_status code) {
+    const std::string keep = g_err;
+    for (void *hs : net->host_streams)
+      if (hs) cudaStreamSynchronize(static_cast<cudaStream_t>(hs));
+    g_err = keep;
+    return code;
+  };
+#define XOD_CUDA_DRAIN(call)                                          \
+  do {                                                                \
+    cudaError_t e_ = (call);                                          \
+    if (e_ != cudaSuccess) return drain(cuda_fail(e_, #call));        \
+  } while (0)
   int slot = 0;
   for (int64_t c0 = 0; c0 < ncol; c0 += cw, slot = (slot + 1) % kHostSlots) {
     const int64_t w = std::min(cw, ncol - c0);
@@ -660,19 +691,45 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
     double *dT = reinterpret_cast<double *>(static_cast<char *>(net->stage) + slot_bytes * slot);
     double *dP = dT + cw, *dJ = dP + cw, *dn = dJ + nph * cw, *dd = dn + ns * cw;
     void *dws = dd + ns * cw;
-    XOD_CUDA(cudaMemcpyAsync(dT, T + c0, wb, cudaMemcpyHostToDevice, s));
-    XOD_CUDA(cudaMemcpyAsync(dP, P + c0, wb, cudaMemcpyHostToDevice, s));
-    if (nph) XOD_CUDA(cudaMemcpy2DAsync(dJ, dp, J + c0, hp, wb, nph, cudaMemcpyHostToDevice, s));
-    XOD_CUDA(cudaMemcpy2DAsync(dn, dp, n + c0, hp, wb, ns, cudaMemcpyHostToDevice, s));
+    XOD_CUDA_DRAIN(cudaMemcpyAsync(dT, T + c0, wb, cudaMemcpyHostToDevice, s));
+    XOD_CUDA_DRAIN(cudaMemcpyAsync(dP, P + c0, wb, cudaMemcpyHostToDevice, s));
+    if (nph) XOD_CUDA_DRAIN(cudaMemcpy2DAsync(dJ, dp, J + c0, hp, wb, nph, cudaMemcpyHostToDevice, s));
+    XOD_CUDA_DRAIN(cudaMemcpy2DAsync(dn, dp, n + c0, hp, wb, ns, cudaMemcpyHostToDevice, s));
     st = xod_source_fused(net, w, cw, dT, dP, dJ, dn, dd, nullptr, nullptr, dws, ws, s);
-    if (st != XOD_OK) return st;
-    XOD_CUDA(cudaMemcpy2DAsync(dndt + c0, hp, dd, dp, wb, ns, cudaMemcpyDeviceToHost, s));
+    if (st != XOD_OK) return drain(st);
+    XOD_CUDA_DRAIN(cudaMemcpy2DAsync(dndt + c0, hp, dd, dp, wb, ns, cudaMemcpyDeviceToHost, s));
   }
+#undef XOD_CUDA_DRAIN
   for (int i = 0; i < kHostSlots; ++i) XOD_CUDA(cudaStreamSynchronize(static_cast<cudaStream_t>(net->host_streams[i])));
   return XOD_OK;
 }
 
 int64_t xod_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+xod_status xod_check_status(const xod_network *net) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  if (net->device < 0) return fail(XOD_ERR_CUDA, "network was created without a CUDA device");
+  DeviceGuard guard(net->device);
+  if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
+  XOD_CUDA(cudaDeviceSynchronize());
+#ifdef XOD_CHECK
+  int line = 0, zero = 0;
+  XOD_CUDA(cudaMemcpyFromSymbol(&line, g_xod_check_line, sizeof line));
+  if (line != 0) {
+    XOD_CUDA(cudaMemcpyToSymbol(g_xod_check_line, &zero, sizeof zero));
+    return fail(XOD_ERR_CUDA, "XOD_CHECK: a table-derived index was out of range at kernel source line " + std::to_string(line));
+  }
+#endif
+  return XOD_OK;
+}
+
+int32_t xod_build_has_checks(void) {
+#ifdef XOD_CHECK
+  return 1;
+#else
+  return 0;
+#endif
+}
 
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches) {
   if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
@@ -695,26 +752,32 @@ xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launch
 
 xod_status xod_probe_fp64_peak(int cuda_device, int32_t iters, double *dfma_per_second) {
   if (!dfma_per_second || iters <= 0) return fail(XOD_ERR_INVALID_ARG, "bad probe arguments");
-  XOD_CUDA(cudaSetDevice(cuda_device));
-  cudaDeviceProp prop;
-  XOD_CUDA(cudaGetDeviceProperties(&prop, cuda_device));
-  const int blocks = prop.multiProcessorCount * 8, threads = 256, inner = 4096;
+  DeviceGuard guard(cuda_device);
+  if (guard.err != cudaSuccess) return cuda_fail(guard.err, "cudaSetDevice");
+  int smc = 0;
+  XOD_CUDA(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, cuda_device));
+  const int blocks = smc * 8, threads = 256, inner = 4096;
   double *out = nullptr;
-  XOD_CUDA(cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)));
-  cudaEvent_t e0, e1;
-  XOD_CUDA(cudaEventCreate(&e0));
-  XOD_CUDA(cudaEventCreate(&e1));
-  k_probe_dfma<<<blocks, threads>>>(out, inner, 1.0000001, 0.9999999);  // warm-up
-  XOD_CUDA(cudaEventRecord(e0));
-  for (int i = 0; i < iters; ++i) k_probe_dfma<<<blocks, threads>>>(out, inner, 1.0000001, 0.9999999);
-  XOD_CUDA(cudaEventRecord(e1));
-  XOD_CUDA(cudaEventSynchronize(e1));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
   float ms = 0;
-  XOD_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(out);
-  XOD_CUDA(cudaGetLastError());
+  cudaError_t e = cudaMalloc(&out, (size_t)blocks * threads * sizeof(double));
+  if (e == cudaSuccess) e = cudaEventCreate(&e0);
+  if (e == cudaSuccess) e = cudaEventCreate(&e1);
+  if (e == cudaSuccess) {
+    k_probe_dfma<<<blocks, threads>>>(out, inner, 1.0000001, 0.9999999);  // warm-up
+    e = cudaEventRecord(e0);
+  }
+  if (e == cudaSuccess) {
+    for (int i = 0; i < iters; ++i) k_probe_dfma<<<blocks, threads>>>(out, inner, 1.0000001, 0.9999999);
+    e = cudaEventRecord(e1);
+  }
+  if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e0) cudaEventDestroy(e0);
+  if (e1) cudaEventDestroy(e1);
+  if (out) cudaFree(out);
+  if (e != cudaSuccess) return cuda_fail(e, "xod_probe_fp64_peak");
   *dfma_per_second = (double)blocks * threads * 16.0 * inner * iters / (ms * 1e-3);
   return XOD_OK;
 }

@@ -27,15 +27,7 @@
 
 #include "xod_internal.h"
 #include "xod_math.cuh"
-
-// Ablation switches for profiling (which phase costs what): compiled in only with -DXOD_ABLATE.
-#ifdef XOD_ABLATE
-#define XOD_DBG(bit) ((a.debug & (bit)) != 0)
-#define XOD_DBG_SHIFT(pos) ((a.debug >> (pos)) & 1)
-#else
-#define XOD_DBG(bit) false
-#define XOD_DBG_SHIFT(pos) 0
-#endif
+#include <xod_cta.cuh>  // CTA primitives (dynamic shared memory, cp.async); resolved through -I csrc
 
 namespace xod {
 
@@ -46,25 +38,12 @@ struct FusedArgs {
   double *out;                // nsplit == 1: dndt [ns][ld]; else partial sums [nsplit][ns][ldp]
   int64_t ldp;                // pitch of the partial sums
   int32_t ntiles, nsplit;
-  int32_t debug;              // ablation switches for profiling (XOD_TUNE_DEBUG); 0 in production
+  int32_t nr, n_photo;        // rows of kf/kr and of J (bounds of the -DXOD_CHECK build)
   double log2_kb;
 };
 
 __device__ __forceinline__ double2 lds2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
 __device__ __forceinline__ double2 ldg2(const unsigned char *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
-#ifndef XOD_EMU
-__device__ __forceinline__ void cp_async16(void *smem, const void *gmem) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
-#else  // tests/kernel_emu: the kernel text compiled as host C++ (a copy completes at once)
-inline void cp_async16(void *smem, const void *gmem) { std::memcpy(smem, gmem, 16); }
-inline void cp_async8(void *smem, const void *gmem) { std::memcpy(smem, gmem, 8); }
-inline void cp_async_wait_all() {}
-#endif
 
 // log2 k_r (UNI/BI) or z (FALLOFF) from the block of interval g
 __device__ __forceinline__ double rev_eval(const unsigned char *blk, int slot16, double c0r /*C0*/, double T,
@@ -85,11 +64,7 @@ __device__ __forceinline__ size_t block_offset(const FusedDev &f, int pp) {
 
 template <bool FROMK>
 __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, FusedArgs a) {
-#ifndef XOD_EMU
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-#else
-  extern unsigned char smem_raw[];  // tests/kernel_emu provides the CTA's shared memory
-#endif
+  unsigned char *smem_raw = cta_dyn_smem();
   double *n_s = reinterpret_cast<double *>(smem_raw);
   double *acc_s = n_s + (size_t)(ns + 1) * kFW;
   double *q_s = acc_s + (size_t)f.n_acc * kFW;
@@ -119,7 +94,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       cLM[tid] = log2(Pc) - a.log2_kb - l2T;  // log2 [M], [M] = P/(k_B T)
       int g = 0;
       for (int k = 0; k < f.n_bp; ++k) g += __ldg(f.bp + k) < Tc;
-      cG[tid] = g;
+      cG[tid] = XOD_IDX(g, f.n_bp + 1);
     }
     // ---- n tile, ones row, zeroed accumulators and zero rows of q
     {
@@ -151,24 +126,22 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       // schedule of this chunk -> shared memory, overlapped with phase A
       {
         const int m0 = __ldg(f.meta_ptr + k), m1 = __ldg(f.meta_ptr + k + 1);
-        for (int u = m0 + tid; u < m1; u += kFWarps * 32) cp_async16(mb + (u - m0), f.meta + u);
+        for (int u = m0 + tid; u < m1; u += kFWarps * 32) cp_async16(mb + XOD_IDX(u - m0, f.meta_cap), f.meta + u);
       }
       // ------------------------------------------------------------ phase A
       const int pp_chunk = k * f.chunk;
 #pragma unroll 1
-      for (int pass_ = 0; pass_ < (f.chunk / kFPass << XOD_DBG_SHIFT(5)); ++pass_) {
-        const int pass = pass_ >> XOD_DBG_SHIFT(5);
+      for (int pass = 0; pass < f.chunk / kFPass; ++pass) {
         const int rbase = pass * kFPass + warp * kFRxnPerWarp;
         const int ppw = pp_chunk + rbase;  // first of the warp's 4 reactions (one segment)
         if (ppw >= f.ph_end) break;        // only padding left
-        if (XOD_DBG(16)) continue;
         double kf0, kf1, kr0, kr1;
         int4 sa;  // species slots as 16-bit indices: r0 r1 | r2 p0 | p1 p2 | J row
         if (FROMK) {
           const int pp = ppw + grp;
-          const unsigned char *b0 = blk0 + block_offset(f, pp) + slot16;
+          const unsigned char *b0 = blk0 + XOD_IDX(block_offset(f, pp), (size_t)f.blk_stride) + slot16;
           sa = __ldg(reinterpret_cast<const int4 *>(b0));
-          const int user = max(__ldg(f.pp_user + pp), 0);  // padding slots read row 0 (their q is never used)
+          const int user = XOD_IDX(max(__ldg(f.pp_user + pp), 0), a.nr);  // padding slots read row 0 (their q is never used)
           const int64_t gc0 = min(col0 + l2, a.ncol - 1), gc1 = min(col0 + l2 + 1, a.ncol - 1);
           const double *kfr = a.kf + (size_t)user * a.ld, *krr = a.kr + (size_t)user * a.ld;
           kf0 = __ldg(kfr + gc0), kf1 = __ldg(kfr + gc1), kr0 = __ldg(krr + gc0), kr1 = __ldg(krr + gc1);
@@ -176,7 +149,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           const bool arr = ppw < f.arr_end;
           const size_t off = arr ? (size_t)(ppw >> 2) * kFBlkArr
                                  : (size_t)f.blk_fo_off + (size_t)((ppw - f.arr_end) >> 2) * kFBlkFo;
-          const unsigned char *b0 = blk0 + off;
+          const unsigned char *b0 = blk0 + XOD_IDX(off, (size_t)f.blk_stride);
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
           const double2 c01 = ldg2(b0 + 2 * 64 + slot16), c2C = ldg2(b0 + 3 * 64 + slot16);
           const double y0 = fma(c2C.x, iT0, fma(c01.y, lT0, c01.x)), y1 = fma(c2C.x, iT1, fma(c01.y, lT1, c01.x));
@@ -188,9 +161,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
           }
           if (arr) {  // UNI, BI
             const unsigned m = max(max(xexp2_mag(y0), xexp2_mag(y1)), max(xexp2_mag(z0), xexp2_mag(z1)));
-            if (XOD_DBG(2)) {
-              kf0 = y0, kf1 = y1, kr0 = z0, kr1 = z1;
-            } else if (m < kExp2FastMax) {
+            if (m < kExp2FastMax) {
               kf0 = xexp2_fast(y0), kf1 = xexp2_fast(y1), kr0 = xexp2_fast(z0), kr1 = xexp2_fast(z1);
             } else {
               kf0 = xexp2_slow(y0), kf1 = xexp2_slow(y1), kr0 = xexp2_slow(z0), kr1 = xexp2_slow(z1);
@@ -209,14 +180,15 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
             kr0 = xexp2(ym0 + z0) * d0, kr1 = xexp2(ym1 + z1) * d1;
           }
         } else {                  // PHOTO
-          const unsigned char *b0 = f.blk + (size_t)f.blk_ph_off + (size_t)((ppw - f.fo_end) >> 2) * kFBlkPh;
+          const unsigned char *b0 = f.blk + XOD_IDX((size_t)f.blk_ph_off + (size_t)((ppw - f.fo_end) >> 2) * kFBlkPh, (size_t)f.blk_stride);
           sa = __ldg(reinterpret_cast<const int4 *>(b0 + slot16));
-          kf0 = a.J[(size_t)sa.w * a.ld + gc0], kf1 = a.J[(size_t)sa.w * a.ld + gc1];
+          const size_t jrow = (size_t)XOD_IDX(sa.w, a.n_photo);
+          kf0 = a.J[jrow * a.ld + gc0], kf1 = a.J[jrow * a.ld + gc1];
           kr0 = kr1 = 0.0;
         }
         // a7: rates of progress (absent slots read the row of ones)
-        const int r0 = sa.x & 0xffff, r1 = (unsigned)sa.x >> 16, r2 = sa.y & 0xffff;
-        const int p0 = (unsigned)sa.y >> 16, p1 = sa.z & 0xffff, p2 = (unsigned)sa.z >> 16;
+        const int r0 = XOD_IDX(sa.x & 0xffff, ns + 1), r1 = XOD_IDX((int)((unsigned)sa.x >> 16), ns + 1), r2 = XOD_IDX(sa.y & 0xffff, ns + 1);
+        const int p0 = XOD_IDX((int)((unsigned)sa.y >> 16), ns + 1), p1 = XOD_IDX(sa.z & 0xffff, ns + 1), p2 = XOD_IDX((int)((unsigned)sa.z >> 16), ns + 1);
         double2 v = lds2(n_l + r0 * kFW);
         double qf0 = kf0 * v.x, qf1 = kf1 * v.y;
         if (r1 != ns) { v = lds2(n_l + r1 * kFW); qf0 *= v.x, qf1 *= v.y; }
@@ -231,8 +203,10 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       __syncthreads();
       // ------------------------------------------------------------ phase B
       const int *hdr = reinterpret_cast<const int *>(mb);
-      const int t_begin = hdr[warp], t_end = XOD_DBG(1) ? t_begin : hdr[warp + 1];
-      const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + hdr[kFWarps + 1]) + grp;
+      const int t_begin = hdr[warp], t_end = XOD_IDX(hdr[warp + 1], f.meta_cap - kFMetaHdr / 4 + 1);
+      const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + XOD_IDX(hdr[kFWarps + 1], f.meta_cap - kFMetaHdr / 4 + 1)) + grp;
+      const int ent_words = (f.meta_cap - kFMetaHdr / 4 - hdr[kFWarps + 1]) * 4;  // XOD_CHECK: words of the entry section
+      (void)ent_words;
       const double *q_l = qb + l2;
       // two warp tasks in flight per iteration (their loads are independent): the dependent
       // chain header -> entry -> q -> FMA is the latency that matters here, not the instruction count
@@ -242,7 +216,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       };
       auto add_row = [&](int row, double s0, double s1) {
         if (row != 0xffff) {
-          double2 *dst = reinterpret_cast<double2 *>(acc_s + (size_t)row * kFW + l2);
+          double2 *dst = reinterpret_cast<double2 *>(acc_s + (size_t)XOD_IDX(row, f.n_acc) * kFW + l2);
           double2 cur = *dst;
           cur.x += s0, cur.y += s1;
           *dst = cur;
@@ -258,23 +232,23 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
         int st = 0;
 #pragma unroll 1
         for (; st < nmin; ++st) {
-          const unsigned xa = ea[st * 4], xb = eb[st * 4];
-          const double2 qa = lds2(q_l + (xa & 0xffffu) * kFW), qc = lds2(q_l + (xb & 0xffffu) * kFW);
+          const unsigned xa = ea[XOD_IDX(ta.x + st * 4 + grp, ent_words) - ta.x - grp], xb = eb[XOD_IDX(tb.x + st * 4 + grp, ent_words) - tb.x - grp];
+          const double2 qa = lds2(q_l + XOD_IDX(xa & 0xffffu, qrows) * kFW), qc = lds2(q_l + XOD_IDX(xb & 0xffffu, qrows) * kFW);
           const double na = __hiloint2double((int)(xa & 0xffff0000u), 0), nb = __hiloint2double((int)(xb & 0xffff0000u), 0);
           a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
           b0 = fma(nb, qc.x, b0), b1 = fma(nb, qc.y, b1);
         }
 #pragma unroll 1
         for (int s2 = st; s2 < ta.y; ++s2) {
-          const unsigned xa = ea[s2 * 4];
-          const double2 qa = lds2(q_l + (xa & 0xffffu) * kFW);
+          const unsigned xa = ea[XOD_IDX(ta.x + s2 * 4 + grp, ent_words) - ta.x - grp];
+          const double2 qa = lds2(q_l + XOD_IDX(xa & 0xffffu, qrows) * kFW);
           const double na = __hiloint2double((int)(xa & 0xffff0000u), 0);
           a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
         }
 #pragma unroll 1
         for (int s2 = st; s2 < tb.y; ++s2) {
-          const unsigned xb = eb[s2 * 4];
-          const double2 qc = lds2(q_l + (xb & 0xffffu) * kFW);
+          const unsigned xb = eb[XOD_IDX(tb.x + s2 * 4 + grp, ent_words) - tb.x - grp];
+          const double2 qc = lds2(q_l + XOD_IDX(xb & 0xffffu, qrows) * kFW);
           const double nb = __hiloint2double((int)(xb & 0xffff0000u), 0);
           b0 = fma(nb, qc.x, b0), b1 = fma(nb, qc.y, b1);
         }
@@ -287,8 +261,8 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
         double a0 = 0.0, a1 = 0.0;
 #pragma unroll 1
         for (int st = 0; st < ta.y; ++st) {
-          const unsigned xa = ea[st * 4];
-          const double2 qa = lds2(q_l + (xa & 0xffffu) * kFW);
+          const unsigned xa = ea[XOD_IDX(ta.x + st * 4 + grp, ent_words) - ta.x - grp];
+          const double2 qa = lds2(q_l + XOD_IDX(xa & 0xffffu, qrows) * kFW);
           const double na = __hiloint2double((int)(xa & 0xffff0000u), 0);
           a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
         }
@@ -300,7 +274,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
     if (tid < kFW) {
       for (int x = 0; x < f.n_extra; ++x) {
         const int er = __ldg(f.extra + 2 * x), sp = __ldg(f.extra + 2 * x + 1);
-        acc_s[sp * kFW + tid] += acc_s[er * kFW + tid];
+        acc_s[XOD_IDX(sp, ns) * kFW + tid] += acc_s[XOD_IDX(er, f.n_acc) * kFW + tid];
       }
     }
     __syncthreads();

@@ -7,6 +7,7 @@
 
 #include "xod_internal.h"
 #include "xod_math.cuh"
+#include <xod_cta.cuh>
 
 namespace xod {
 
@@ -302,9 +303,9 @@ __global__ void __launch_bounds__(256) k_jacobian(DevTables d, int64_t ncol, int
     for (int64_t t = t0; t < t1; ++t) {
       const int4 tm = __ldg(reinterpret_cast<const int4 *>(d.jac_terms + t));
       const double *k = tm.x < 0 ? kr : kf;
-      double v = (double)__int_as_float(tm.w) * k[(size_t)(tm.x & 0x7fffffff) * ld + cc];
-      if (tm.y >= 0) v *= n[(size_t)tm.y * ld + cc];
-      if (tm.z >= 0) v *= n[(size_t)tm.z * ld + cc];
+      double v = (double)__int_as_float(tm.w) * k[(size_t)XOD_IDX(tm.x & 0x7fffffff, d.nr) * ld + cc];
+      if (tm.y >= 0) v *= n[(size_t)XOD_IDX(tm.y, d.ns) * ld + cc];
+      if (tm.z >= 0) v *= n[(size_t)XOD_IDX(tm.z, d.ns) * ld + cc];
       acc += v;
     }
     if (valid) jac[(size_t)e * ld + c] = acc;

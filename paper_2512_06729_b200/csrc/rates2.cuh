@@ -12,13 +12,15 @@
 
 #include "xod_internal.h"
 #include "xod_math.cuh"
+#include <xod_cta.cuh>
 
 namespace xod {
 
 
 __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, int64_t ld, const double *__restrict__ T,
                                                      const double *__restrict__ P, const double *__restrict__ J,
-                                                     double *__restrict__ kf, double *__restrict__ kr, double log2_kb, int slice) {
+                                                     double *__restrict__ kf, double *__restrict__ kr, double log2_kb, int slice,
+                                                     int nr, int n_photo /* rows of kf/kr and of J: bounds of the -DXOD_CHECK build */) {
   const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c - (threadIdx.x & 31) >= ncol) return;  // whole warp past the end
   const bool valid = c < ncol;
@@ -28,7 +30,7 @@ __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, i
   const double lM = log2(P[gc]) - log2_kb - l2T;  // log2 [M], [M] = P/(k_B T)
   int g = 0;
   for (int k = 0; k < f.n_bp; ++k) g += __ldg(f.bp + k) < Tc;
-  const unsigned char *blkg = f.blk + (size_t)g * f.blk_stride;
+  const unsigned char *blkg = f.blk + (size_t)XOD_IDX(g, f.n_bp + 1) * f.blk_stride;
   const int p0 = blockIdx.y * slice, p1 = min(p0 + slice, f.ph_end);
 #pragma unroll 2
   for (int pp = p0; pp < p1; ++pp) {
@@ -38,8 +40,8 @@ __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, i
     if (pp < f.fo_end) {
       const bool arr = pp < f.arr_end;
       const unsigned char *b = blkg + slot16 +
-                               (arr ? (size_t)(pp >> 2) * kFBlkArr
-                                    : (size_t)f.blk_fo_off + (size_t)((pp - f.arr_end) >> 2) * kFBlkFo);
+                               XOD_IDX(arr ? (size_t)(pp >> 2) * kFBlkArr
+                                           : (size_t)f.blk_fo_off + (size_t)((pp - f.arr_end) >> 2) * kFBlkFo, (size_t)f.blk_stride);
       const double2 c01 = __ldg(reinterpret_cast<const double2 *>(b + 2 * 64));
       const double2 c2C = __ldg(reinterpret_cast<const double2 *>(b + 3 * 64));
       const double2 c12 = __ldg(reinterpret_cast<const double2 *>(b + 4 * 64));
@@ -64,13 +66,14 @@ __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, i
         vr = xexp2(ym + z) * den;
       }
     } else {
-      const unsigned char *b = blkg + (size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh + slot16;
-      const int jrow = __ldg(reinterpret_cast<const int *>(b) + 3);
+      const unsigned char *b = blkg + XOD_IDX((size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh, (size_t)f.blk_stride) + slot16;
+      const int jrow = XOD_IDX(__ldg(reinterpret_cast<const int *>(b) + 3), n_photo);
       vf = J[(size_t)jrow * ld + gc];
     }
     if (valid && user >= 0) {  // user < 0: padding slot
-      if (kf) kf[(size_t)user * ld + c] = vf;
-      if (kr) kr[(size_t)user * ld + c] = vr;
+      const size_t row = (size_t)XOD_IDX(user, nr);
+      if (kf) kf[row * ld + c] = vf;
+      if (kr) kr[row * ld + c] = vr;
     }
   }
 }

@@ -166,8 +166,7 @@ struct xod_network {
   xod::FusedDev fd{};
   int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
   int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
-  int sm_count = 148;
-  int64_t debug = 0;
+  int sm_count = 148;       // replaced by the device attribute at create
   int device = -1;
   std::vector<void *> dev_allocs;
   int64_t chunk_cols = 0;  // 0 = default

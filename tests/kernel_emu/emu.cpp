@@ -98,6 +98,7 @@ int emu_source_fused(const xod_network_desc *d, int64_t ncol, int64_t ld, const 
   a.nsplit = std::max(1, std::min(nsplit, (int)fd.nchunk));
   a.log2_kb = kLog2Kb;
   a.ldp = (ncol + 31) / 32 * 32;
+  a.nr = h.nr, a.n_photo = h.n_photo;
   std::vector<double> part((size_t)a.nsplit * h.ns * a.ldp);
   a.out = a.nsplit == 1 ? dndt : part.data();
   const int ns = h.ns;
@@ -117,7 +118,7 @@ int emu_rate_coeffs(const xod_network_desc *d, int64_t ncol, int64_t ld, const d
   FusedDev fd;
   if (!pack(d, h, fd) || ncol <= 0) return 1;
   run_grid((unsigned)((ncol + 255) / 256), (unsigned)((fd.ph_end + slice - 1) / slice), 256, false,
-           [&] { k_rate_coeffs(fd, ncol, ld, T, P, J, kf, kr, kLog2Kb, slice); });
+           [&] { k_rate_coeffs(fd, ncol, ld, T, P, J, kf, kr, kLog2Kb, slice, h.nr, h.n_photo); });
   return 0;
 }
 

@@ -19,13 +19,13 @@ CSRC = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
 LIB = os.path.join(EMU_DIR, "libxod_emu.so")
 SOURCES = [os.path.join(EMU_DIR, "emu.cpp"), os.path.join(CSRC, "pack.cpp"), os.path.join(CSRC, "pack_fused.cpp")]
 DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "xod_math.cuh", "xod_internal.h")] + [
-    os.path.join(EMU_DIR, "shim", "cuda_runtime.h")]
+    os.path.join(EMU_DIR, "shim", "cuda_runtime.h"), os.path.join(EMU_DIR, "shim", "xod_cta.cuh")]
 
 
 @pytest.fixture(scope="module")
 def emu():
     if not os.path.exists(LIB) or any(os.path.getmtime(d) > os.path.getmtime(LIB) for d in DEPS):
-        subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-shared", "-fPIC", "-DXOD_EMU",
+        subprocess.run(["g++", "-std=c++20", "-O1", "-pthread", "-shared", "-fPIC",
                         "-I" + os.path.join(EMU_DIR, "shim"), "-o", LIB] + SOURCES, check=True)
     return C.CDLL(LIB)
 
@@ -193,7 +193,7 @@ def test_fused_kernel_source_is_race_free_under_thread_sanitizer():
         pytest.skip("libtsan not available")
     lib = os.path.join(EMU_DIR, "libxod_emu_tsan.so")
     if not os.path.exists(lib) or any(os.path.getmtime(d) > os.path.getmtime(lib) for d in DEPS):
-        subprocess.run(["g++", "-std=c++20", "-O1", "-g", "-fsanitize=thread", "-pthread", "-shared", "-fPIC", "-DXOD_EMU",
+        subprocess.run(["g++", "-std=c++20", "-O1", "-g", "-fsanitize=thread", "-pthread", "-shared", "-fPIC",
                         "-I" + os.path.join(EMU_DIR, "shim"), "-o", lib] + SOURCES, check=True)
     env = dict(os.environ, LD_PRELOAD=tsan, TSAN_OPTIONS="halt_on_error=0 report_signal_unsafe=0 exitcode=0")
     out = subprocess.run([os.sys.executable, "-c", TSAN_CHILD, ROOT, lib], capture_output=True, text=True, env=env,
