@@ -26,6 +26,15 @@ def xod():
 _handles = {}
 
 
+@pytest.fixture(autouse=True)
+def _device_clean_after_each_test(xod):
+    """After every test: synchronise and, in the bounds-checked build (XOD_CHECK=1), fail if a kernel
+    saw an out-of-range table index (the check build clamps and records instead of faulting)."""
+    yield
+    for h in _handles.values():
+        h.check_status()
+
+
 def handle(xod, network, cfg):
     key = 3 if cfg in (3, 4, 5) else cfg
     if key not in _handles:
@@ -299,12 +308,14 @@ def test_ragged_sizes_and_pitches(xod, oracle, network, ncol, ld):
 
 
 def test_chunk_boundaries_do_not_change_results(xod, network):
-    """The column-chunk pipeline must be invisible: 64-column chunks == one chunk, bit for bit."""
+    """The column-chunk pipeline (multi-kernel path: col0 > 0 in k_prologue / k_rates / k_source) must be
+    invisible: 64-column chunks == one chunk, bit for bit."""
     net = network(3)
     atm = atmosphere(3, net)
     outs = []
     for chunk in (0, 64):
         h = xod.Network(net, device=0)
+        h.tune(xod.XOD_TUNE_FUSED_KERNEL, 0)
         h.tune(xod.XOD_TUNE_CHUNK_COLS, chunk)
         ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
         d0 = G.empty(net.n_species, atm.ld)
