@@ -603,3 +603,97 @@ def config_atmosphere(cfg, net, n_atm=None):
     if cfg == 5:
         return make_atmosphere(2005, net, n_atm or 64, 150)
     raise ValueError("config must be 1..5")
+
+
+# --------------------------------------------------------------------------- the edge-case network
+
+def edge_network(seed=1099):
+    """A mid-size network that holds every reaction shape the paper allows but configs 1-5 do not
+    draw (the parity tests run it through every kernel):
+      * irreversible thermal reactions of all three thermal types (one-way steps, PAPER.md:408);
+      * pure Lindemann falloff, Fc = 1 (Eq. 12 exactly, PAPER.md:157);
+      * a species three times on one side, nu = -3 and nu = +3 (Eq. 13 allows three, PAPER.md:225);
+      * an ion / electron pair with the charge carried as a signed extra "element" (PAPER.md:363);
+      * a species that takes part in no reaction (empty CSR row);
+      * Kooij (t_ref = 300) and modified-Arrhenius (t_ref = 1) forms mixed.
+    Structure only; parameters come from the same distributions as the configs."""
+    base = make_network(seed, _ELEMENTS[2], 60, 400, name="edge")
+    rng = np.random.default_rng(seed + 1)
+    ns0, ne0, nr0 = base.n_species, base.n_elements, base.n_reactions
+    comp = np.zeros((ns0 + 4, ne0 + 1), dtype=np.int32)          # last column: charge
+    comp[:ns0, :ne0] = base.composition
+    used = np.unique(np.concatenate([base.reactants.ravel(), base.products.ravel()]))
+    a = int(used[used >= 0][0])                                  # a species the sampler uses
+    x3, ion, el, lone = ns0, ns0 + 1, ns0 + 2, ns0 + 3
+    comp[x3, :ne0] = 3 * base.composition[a]
+    comp[ion, :ne0] = base.composition[a]
+    comp[ion, ne0] = +1
+    comp[el, ne0] = -1
+    comp[lone, :ne0] = base.composition[a]                       # an isomer no reaction touches
+    lo4, hi4, tm4 = _make_nasa(rng, 4)
+    tm4 = np.array([300.0, 500.0, 700.0, 1000.0])                # every junction temperature of SURVEY T3 occurs
+    extra = [  # (type, reactants, products, reversible, Fc)
+        (BI, [a, a, a], [x3], 1, 1.0),          # nu_a = -3
+        (UNI, [x3], [a, a, a], 0, 1.0),         # nu_a = +3, one-way
+        (PHOTO, [a], [ion, el], 0, 1.0),        # photo-ionisation
+        (BI, [ion, el], [a], 1, 1.0),           # recombination, reverse by detailed balance
+        (FALLOFF, [ion, el], [a], 0, 1.0),      # three-body recombination, pure Lindemann, one-way
+    ]
+    nr = nr0 + len(extra)
+    rtype = np.concatenate([base.type, np.array([e[0] for e in extra], dtype=np.int32)])
+    reactants = -np.ones((nr, 3), dtype=np.int32)
+    products = -np.ones((nr, 3), dtype=np.int32)
+    reactants[:nr0], products[:nr0] = base.reactants, base.products
+    for k, (_, lhs, rhs, _, _) in enumerate(extra):
+        reactants[nr0 + k, :len(lhs)] = lhs
+        products[nr0 + k, :len(rhs)] = rhs
+        assert _check_balance(comp, lhs, rhs)
+    reversible = np.concatenate([base.reversible, np.array([e[3] for e in extra], dtype=np.uint8)])
+    thermal = rtype != PHOTO
+    one_way = thermal & (rng.uniform(size=nr) < 1.0 / 3.0)
+    one_way[nr0:] = False
+    reversible[one_way] = 0
+    fc = np.concatenate([base.troe_fc, np.array([e[4] for e in extra])])
+    is_fo = rtype == FALLOFF
+    fc[is_fo & (rng.uniform(size=nr) < 0.25)] = 1.0
+    fc[nr0:] = [e[4] for e in extra]
+    t_ref = np.where(thermal & (rng.uniform(size=nr) < 1.0 / 3.0), 300.0, 1.0)
+
+    def draw3(n_rows, a_lo, a_hi):
+        return np.stack([_loguniform(rng, a_lo, a_hi, size=n_rows), rng.uniform(-3.0, 3.0, size=n_rows),
+                         rng.uniform(0.0, 40000.0, size=n_rows)], axis=1)
+
+    arrh = np.concatenate([base.arrh, draw3(len(extra), 1e-20, 1e-9)])
+    arrh[nr0 + 1, 0] = _loguniform(rng, 1e6, 1e16)               # the unimolecular one
+    arrh[rtype == PHOTO] = 0.0
+    arrh_low = np.concatenate([base.arrh_low, draw3(len(extra), 1e-36, 1e-26)])
+    arrh_low[~is_fo] = 0.0
+    perm = rng.permutation(nr)                                   # the added reactions are not left at the end
+    assert {UNI, BI, FALLOFF} <= set(rtype[reversible == 0].tolist())
+    return Network(
+        element_names=list(base.element_names) + ["charge"], composition=comp,
+        nasa_lo=np.concatenate([base.nasa_lo, lo4]), nasa_hi=np.concatenate([base.nasa_hi, hi4]),
+        t_mid=np.concatenate([base.t_mid, tm4]), type=rtype[perm], reactants=reactants[perm],
+        products=products[perm], reversible=reversible[perm], arrh=arrh[perm], arrh_low=arrh_low[perm],
+        troe_fc=fc[perm], t_ref=t_ref[perm],
+        meta={"name": "edge", "seed": seed, "triple": a, "x3": x3, "ion": ion, "electron": el, "lone": lone})
+
+
+def edge_atmosphere(net, seed=2099, n_layers=75):
+    """One atmosphere for `edge_network` whose columns include: T exactly on every thermo breakpoint
+    t_mid and one ulp below and above it (reading T3: T <= t_mid takes the low set), a cold column
+    (k_r beyond the double range, reading R5), a species that is zero everywhere, a column that is
+    zero everywhere, and a negative density (reading Q2: processed arithmetically)."""
+    atm = make_atmosphere(seed, net, 1, n_layers)
+    c = 1
+    for tm in np.unique(net.t_mid):
+        for T in (np.nextafter(tm, 0.0), tm, np.nextafter(tm, 1e9)):
+            atm.T[c] = T
+            c += 2                                               # leave ordinary columns in between
+    assert c < atm.ncol - 8
+    atm.T[c] = 170.0
+    atm.n[5, :] = 0.0
+    atm.n[:, c + 2] = 0.0
+    atm.n[7, c + 4] = -atm.n[7, c + 4]
+    atm.meta.update(cold=c, zero_species=5, zero_column=c + 2, negative=(7, c + 4))
+    return atm

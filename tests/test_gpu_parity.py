@@ -216,7 +216,7 @@ def test_source_fused_config4_batch(xod, oracle, network):
     non-finite k_r excluded by reading R5 (their count is reported, and must be > 0 here)."""
     net = network(4)
     h = handle(xod, network, 4)
-    atm = atmosphere(4, net, n_atm=9)                 # 1350 columns: 2 chunks of 1024, ragged
+    atm = atmosphere(4, net, n_atm=9)                 # 1350 columns: 84 full tiles and a ragged one (6 columns)
     okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
     want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
     ns, ld = net.n_species, atm.ld
@@ -346,35 +346,41 @@ def _gather_columns(atm, cols):
     return atm.T[cols].copy(), atm.P[cols].copy(), atm.J[:, cols].copy(), atm.n[:, cols].copy()
 
 
-def test_full_size_config4_sampled_columns(xod, oracle, network):
+def test_full_size_config4_whole_batch(xod, oracle, network):
     """BASELINE config 4 at full size (256 x 150 = 38 400 columns) in the launch configuration
-    bench.py times (one xod_source_fused call), checked on sampled columns the oracle evaluates one
-    by one: tile edges, the first and last tile, random interior columns."""
+    bench.py times (one xod_source_fused call), every column against the oracle (about a minute of
+    oracle time); columns with k_r beyond the double range are excluded by reading R5 and counted."""
     net = network(4)
     h = handle(xod, network, 4)
     atm = atmosphere(4, net)
     assert atm.ncol == 38400
     ws = G.workspace(h.source_fused_workspace_bytes(atm.ncol))
-    d0 = G.empty(net.n_species, atm.ld)
-    h.source_fused(atm.ncol, atm.ld, G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n), d0, workspace=ws)
+    d0, p0, l0 = G.empty(net.n_species, atm.ld), G.empty(net.n_species, atm.ld), G.empty(net.n_species, atm.ld)
+    dT, dP, dJ, dn = G.dev(atm.T), G.dev(atm.P), G.dev(atm.J), G.dev(atm.n)
+    h.source_fused(atm.ncol, atm.ld, dT, dP, dJ, dn, d0, workspace=ws)
     got = G.host(d0)
-    rng = np.random.default_rng(4)
-    cols = np.unique(np.concatenate([[0, 1, 15, 16, 17, 31, 32, atm.ncol - 17, atm.ncol - 16, atm.ncol - 1],
-                                     rng.integers(0, atm.ncol, size=54)]))
-    T, P, J, n = _gather_columns(atm, cols)
-    okf, okr = oracle.rate_coeffs(net, T, P, J)
-    want, wp, wl = oracle.source(net, okf, okr, n)
-    ok = G.finite_columns(okf, okr, want, wp, wl)
-    assert ok.sum() >= cols.size // 2
-    G.check_sum(got[:, cols], want, wp + wl, np.flatnonzero(ok), "full-size fused dn/dt (sampled)")
-    assert element_residual(net, got[:, cols], wp + wl, np.flatnonzero(ok)) <= 1e-13
-    # a property that holds at any size: columns whose inputs are finite give finite-or-inf results, never NaN
-    # unless an overflowed k_r met a zero density (inf x 0), which the oracle reproduces on the sampled columns
-    nan_cols = np.isnan(got[:, cols]).any(axis=0)
-    assert np.array_equal(nan_cols, np.isnan(want).any(axis=0))
+    h.source_fused(atm.ncol, atm.ld, dT, dP, dJ, dn, d0, p0, l0, workspace=ws)
+    got_pl, gp, gl = G.host(d0), G.host(p0), G.host(l0)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    c = slice(0, atm.ncol)
+    ok = G.finite_columns(okf[:, c], okr[:, c], want[:, c], wp[:, c], wl[:, c])
+    cols = np.flatnonzero(ok)
+    scale = wp + wl
+    worst = G.check_sum(got, want, scale, cols, "full-size fused dn/dt")
+    res = element_residual(net, got, scale, cols)
+    print("config 4, all %d columns: %d excluded by R5; worst |err|/scale = %.2e; element residual %.2e"
+          % (atm.ncol, atm.ncol - cols.size, worst, res))
+    assert 0 < atm.ncol - cols.size < atm.ncol // 2
+    assert res <= 1e-13
+    G.check_sum(got_pl, want, scale, cols, "full-size fused dn/dt (P/L variant)")
+    G.check_sum(gp, wp, scale, cols, "full-size fused P")
+    G.check_sum(gl, wl, scale, cols, "full-size fused L")
+    # excluded columns: NaN only where the oracle has NaN (an overflowed k_r met a zero density)
+    assert np.array_equal(np.isnan(got[:, c]).any(axis=0), np.isnan(want[:, c]).any(axis=0))
 
 
-def test_full_size_config5_jacobian_sampled_columns(xod, oracle, network):
+def test_full_size_config5_jacobian_whole_atmospheres(xod, oracle, network):
     """BASELINE config 5 at full size (64 x 150 = 9 600 columns): rate coefficients, dn/dt and
     Jacobian values, checked on sampled columns."""
     net = network(5)
@@ -389,16 +395,18 @@ def test_full_size_config5_jacobian_sampled_columns(xod, oracle, network):
     h.jacobian(atm.ncol, ld, kf, kr, n, jac)
     d0 = G.empty(ns, ld)
     h.source(atm.ncol, ld, kf, kr, n, d0, workspace=G.workspace(h.source_workspace_bytes(atm.ncol)))
-    cols = np.array([0, 31, 32, 4799, 9568, 9599])
+    # two whole atmospheres (the first and one from the middle) plus the edges of the last tiles
+    cols = np.unique(np.concatenate([np.arange(150), np.arange(31 * 150, 32 * 150), [9567, 9568, 9583, 9584, 9599]]))
     Tc, Pc, Jc, nc = _gather_columns(atm, cols)
     okf, okr = oracle.rate_coeffs(net, Tc, Pc, Jc)
     G.check_k(G.host(kf)[:, cols], okf, "full-size k_f")
     G.check_k(G.host(kr)[:, cols], okr, "full-size k_r")
     rp, col = h.jac_pattern()
     wj, sj = oracle.jacobian(net, okf, okr, nc, rp, col)
-    G.check_sum(G.host(jac)[:, cols], wj, sj, np.arange(cols.size), "full-size Jacobian (sampled)")
+    wj_worst = G.check_sum(G.host(jac)[:, cols], wj, sj, np.arange(cols.size), "full-size Jacobian (%d columns)" % cols.size)
     want, wp, wl = oracle.source(net, okf, okr, nc)
-    G.check_sum(G.host(d0)[:, cols], want, wp + wl, np.arange(cols.size), "full-size dn/dt (sampled)")
+    wd = G.check_sum(G.host(d0)[:, cols], want, wp + wl, np.arange(cols.size), "full-size dn/dt (sampled)")
+    print("config 5, %d of %d columns: worst |err|/scale Jacobian %.2e, dn/dt %.2e" % (cols.size, atm.ncol, wj_worst, wd))
 
 
 def test_reaction_split_path_matches_single_pass(xod, oracle, network):
@@ -472,3 +480,118 @@ def test_host_entry_point_pipelines_column_chunks(xod, oracle, network):
     T, P, J, n = _gather_columns(atm, cols)
     want, wp, wl = oracle.source_from_state(net, T, P, J, n)
     G.check_sum(out[:, cols], want, wp + wl, np.arange(cols.size), "host pipeline dn/dt (sampled)")
+
+
+# ------------------------------------------------------------------------------- the edge-case network
+@pytest.fixture(scope="module")
+def edge(xod, oracle):
+    from paper_2512_06729_b200 import synth
+    net = synth.edge_network()
+    atm = synth.edge_atmosphere(net)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    c = slice(0, atm.ncol)
+    cols = np.flatnonzero(G.finite_columns(okf[:, c], okr[:, c], want[:, c], wp[:, c], wl[:, c]))
+    h = xod.Network(net, device=0)
+    _handles["edge"] = h
+    return net, atm, h, okf, okr, want, wp, wl, cols
+
+
+def test_edge_network_rate_coefficients(xod, edge):
+    """Irreversible thermal reactions (k_r = 0 exactly), Fc = 1 (Eq. 12), Kooij forms, ions, and T on /
+    one ulp beside every thermo breakpoint (reading T3) -- through k_rate_coeffs and the multi-kernel pipeline."""
+    net, atm, h, okf, okr, *_ = edge
+    c = slice(0, atm.ncol)
+    for fused in (1, 0):
+        h.tune(xod.XOD_TUNE_FUSED_KERNEL, fused)
+        kf, kr = run_rate_coeffs(h, atm)
+        wf = G.check_k(kf[:, c], okf[:, c], "edge k_f (fused tables %d)" % fused)
+        wr = G.check_k(kr[:, c], okr[:, c], "edge k_r (fused tables %d)" % fused)
+        assert np.all(kr[net.reversible == 0][:, c] == 0.0)
+        print("edge network k (single-kernel %d): worst relative error k_f %.2e, k_r %.2e" % (fused, wf, wr))
+    h.tune(xod.XOD_TUNE_FUSED_KERNEL, 1)
+    assert np.isinf(okr[:, c]).any()
+
+
+def test_edge_network_source_all_paths(xod, edge):
+    """nu = +-3, an empty CSR row, a zero species, a zero column, a negative density: xod_source and
+    xod_source_fused, with and without P/L, single-kernel and multi-kernel, reaction-split or not."""
+    net, atm, h, okf, okr, want, wp, wl, cols = edge
+    ns, ld, ncol = net.n_species, atm.ld, atm.ncol
+    scale = wp + wl
+    dT, dP, dJ, dn, dkf, dkr = (G.dev(a) for a in (atm.T, atm.P, atm.J, atm.n, okf, okr))
+    ws = G.workspace(max(h.source_fused_workspace_bytes(ncol), h.source_workspace_bytes(ncol)) + (64 << 20))
+    for fused, split in ((1, 0), (1, 2), (0, 0)):
+        h.tune(xod.XOD_TUNE_FUSED_KERNEL, fused)
+        h.tune(xod.XOD_TUNE_SPLIT, split)
+        for pl in (False, True):
+            for stored in (False, True):
+                d0 = G.empty(ns, ld)
+                p0, l0 = (G.empty(ns, ld), G.empty(ns, ld)) if pl else (None, None)
+                if stored:
+                    h.source(ncol, ld, dkf, dkr, dn, d0, p0, l0, workspace=ws)
+                else:
+                    h.source_fused(ncol, ld, dT, dP, dJ, dn, d0, p0, l0, workspace=ws)
+                what = "edge dn/dt (single-kernel %d, split %d, P/L %d, stored k %d)" % (fused, split, pl, stored)
+                got = G.host(d0)
+                worst = G.check_sum(got, want, scale, cols, what)
+                G.check_sum_entries(got, want, scale, ncol, what + " entry-wise")
+                assert np.all(np.isnan(got[:, ncol:])), what
+                assert np.all(got[net.meta["lone"], cols] == 0.0) and np.all(got[:, atm.meta["zero_column"]] == 0.0)
+                assert element_residual(net, got, scale, cols) <= 1e-13, what
+                if pl:
+                    G.check_sum(G.host(p0), wp, scale, cols, what + " P")
+                    G.check_sum(G.host(l0), wl, scale, cols, what + " L")
+                print("%s: worst |err|/scale %.2e" % (what, worst))
+    h.tune(xod.XOD_TUNE_FUSED_KERNEL, 1)
+    h.tune(xod.XOD_TUNE_SPLIT, 0)
+
+
+def test_edge_network_jacobian_and_thermo(xod, oracle, edge):
+    net, atm, h, okf, okr, want, wp, wl, cols = edge
+    ncol, ld = atm.ncol, atm.ld
+    okr_f = np.where(np.isfinite(okr), okr, 0.0)      # finite inputs for the dense oracle; those columns are not compared
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr_f, atm.n, rp, col, ncol)
+    jac = G.empty(h.nnz_jac, ld)
+    h.jacobian(ncol, ld, G.dev(okf), G.dev(okr_f), G.dev(atm.n), jac)
+    worst = G.check_sum(G.host(jac), wj, sj, cols, "edge Jacobian")
+    print("edge network Jacobian: worst |err|/scale %.2e" % worst)
+    outs = [G.empty(net.n_species, ld) for _ in range(4)]
+    h.thermo(ncol, ld, G.dev(atm.T), *outs)
+    for got, w, s in zip(outs, oracle.thermo(net, atm.T, ncol), thermo_scale(net, atm.T)):
+        assert np.all(np.abs(G.host(got)[:, :ncol] - w[:, :ncol]) <= G.TOL_THERMO * s[:, :ncol])
+
+
+def test_production_and_loss_over_several_column_chunks(xod, oracle, network):
+    """P and L on 2 500 columns of the config-4 family: several chunks / rounds of tiles with a ragged tail,
+    for xod_source and xod_source_fused, single-kernel and multi-kernel (64-column chunks, col0 > 0)."""
+    net = network(4)
+    atm = atmosphere(4, net, n_atm=17)
+    atm.ncol = 2500
+    ncol, ld, ns = atm.ncol, atm.ld, net.n_species
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    c = slice(0, ncol)
+    cols = np.flatnonzero(G.finite_columns(okf[:, c], okr[:, c], want[:, c], wp[:, c], wl[:, c]))
+    scale = wp + wl
+    okr_f = np.where(np.isfinite(okr), okr, 0.0)
+    dT, dP, dJ, dn, dkf, dkr = (G.dev(a) for a in (atm.T, atm.P, atm.J, atm.n, okf, okr_f))
+    for fused, chunk in ((1, 0), (0, 64)):
+        h = xod.Network(net, device=0)
+        h.tune(xod.XOD_TUNE_FUSED_KERNEL, fused)
+        h.tune(xod.XOD_TUNE_CHUNK_COLS, chunk)
+        ws = G.workspace(max(h.source_fused_workspace_bytes(ncol), h.source_workspace_bytes(ncol)))
+        for stored in (False, True):
+            d0, p0, l0 = G.empty(ns, ld), G.empty(ns, ld), G.empty(ns, ld)
+            if stored:
+                h.source(ncol, ld, dkf, dkr, dn, d0, p0, l0, workspace=ws)
+            else:
+                h.source_fused(ncol, ld, dT, dP, dJ, dn, d0, p0, l0, workspace=ws)
+            what = "P/L over chunks (single-kernel %d, stored k %d)" % (fused, stored)
+            G.check_sum(G.host(d0), want, scale, cols, what + " dn/dt")
+            G.check_sum(G.host(p0), wp, scale, cols, what + " P")
+            G.check_sum(G.host(l0), wl, scale, cols, what + " L")
+            assert np.all(np.isnan(G.host(d0)[:, ncol:])) and np.all(np.isnan(G.host(p0)[:, ncol:]))
+        h.check_status()
+        h.close()

@@ -11,6 +11,7 @@ import numpy as np
 import pytest
 
 from conftest import ROOT
+import gpu_common as G
 
 from paper_2512_06729_b200 import binding
 
@@ -165,6 +166,101 @@ def test_multi_kernel_pipeline_sources_match_oracle(emu, oracle, network, cfg):
                                         ptr(kf), ptr(kr), C.c_int(16)) == 0
     assert np.all(np.abs(kf[:, :ncol] - okf[:, :ncol]) <= 1e-12 * np.abs(okf[:, :ncol]))
     assert np.all(np.abs(kr[:, :ncol] - okr[:, :ncol]) <= 1e-12 * np.abs(okr[:, :ncol]))
+
+
+# ------------------------------------------------------------------------------- the edge-case network
+@pytest.fixture(scope="module")
+def edge(oracle):
+    """synth.edge_network / edge_atmosphere with the oracle's results (shared by the tests below)."""
+    from paper_2512_06729_b200 import synth
+    net = synth.edge_network()
+    atm = synth.edge_atmosphere(net)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, atm.ncol)
+    c = slice(0, atm.ncol)
+    fin = G.finite_columns(okf[:, c], okr[:, c], want[:, c], wp[:, c], wl[:, c])
+    assert 0 < (~fin).sum() <= 8, "only the cold columns (170 K, 300 K) hold k_r beyond the double range (reading R5)"
+    return net, atm, okf, okr, want, wp, wl, np.flatnonzero(fin)
+
+
+def test_edge_network_has_every_shape():
+    from paper_2512_06729_b200 import synth
+    net = synth.edge_network()
+    h = binding.Network(net, device=-1)
+    h.selfcheck()
+    rp, rxn, nu = h.source_csr()
+    assert nu.min() == -3 and nu.max() == 3
+    assert rp[net.meta["lone"] + 1] == rp[net.meta["lone"]], "a species in no reaction has an empty CSR row"
+    irr = net.reversible == 0
+    assert {0, 1, 2} <= set(net.type[irr].tolist())
+    assert np.any((net.type == 2) & (net.troe_fc == 1.0)) and np.any((net.type == 2) & (net.troe_fc < 1.0))
+    assert np.any(net.t_ref == 300.0) and np.any(net.t_ref == 1.0)
+    assert net.composition[net.meta["ion"], -1] == 1 and net.composition[net.meta["electron"], -1] == -1
+    atm = synth.edge_atmosphere(net)
+    for tm in np.unique(net.t_mid):
+        assert np.any(atm.T[:atm.ncol] == tm) and np.any(atm.T[:atm.ncol] == np.nextafter(tm, 0)) \
+            and np.any(atm.T[:atm.ncol] == np.nextafter(tm, 1e9))
+
+
+@pytest.mark.parametrize("grid,nsplit,fromk", [(2, 1, False), (3, 2, False), (2, 1, True)])
+def test_edge_network_fused_kernel_source(emu, edge, grid, nsplit, fromk):
+    """k_fused on irreversible reactions (C0 = -inf), Fc = 1, nu = +-3, ions, an empty CSR row, Kooij
+    forms, and columns sitting exactly on / one ulp beside every thermo breakpoint inside a tile."""
+    net, atm, okf, okr, want, wp, wl, cols = edge
+    kw = dict(kf=np.ascontiguousarray(okf), kr=np.ascontiguousarray(okr)) if fromk else {}
+    got = run_fused(emu, net, atm, atm.ncol, grid=grid, nsplit=nsplit, **kw)
+    worst = G.check_sum(got, want, wp + wl, cols, "emulated k_fused, edge network")
+    # columns with some overflowing k_r (T = 300 K -+ 1 ulp among them): every entry they do not reach still matches
+    w2, skipped = G.check_sum_entries(got, want, wp + wl, atm.ncol, "emulated k_fused, edge network, entry-wise")
+    assert skipped > 0
+    assert np.all(np.isnan(got[:, atm.ncol:]))
+    assert np.all(got[net.meta["lone"], cols] == 0.0)
+    zc = atm.meta["zero_column"]
+    assert np.all(got[:, zc] == 0.0), "a column of zero densities gives exact zeros"
+    print("edge network, k_fused(fromk=%s, split %d): worst |err|/scale = %.2e on %d columns" % (fromk, nsplit, worst, cols.size))
+
+
+def test_edge_network_rate_coefficient_kernel_source(emu, edge):
+    net, atm, okf, okr, *_ = edge
+    d, keep = descriptor(net)
+    kf = np.full((net.n_reactions, atm.ld), np.nan)
+    kr = np.full((net.n_reactions, atm.ld), np.nan)
+    assert emu.emu_rate_coeffs(C.byref(d), C.c_int64(atm.ncol), C.c_int64(atm.ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                               ptr(kf), ptr(kr), C.c_int(12)) == 0
+    c = slice(0, atm.ncol)
+    wf = G.check_k(kf[:, c], okf[:, c], "emulated k_rate_coeffs k_f, edge network")
+    wr = G.check_k(kr[:, c], okr[:, c], "emulated k_rate_coeffs k_r, edge network")
+    irr = net.reversible == 0
+    assert np.all(kr[irr][:, c] == 0.0), "irreversible reactions have k_r = 0 exactly"
+    assert np.isinf(okr[:, c]).any(), "the cold column overflows (reading R5)"
+    print("edge network, k_rate_coeffs: worst relative error k_f %.2e, k_r %.2e" % (wf, wr))
+
+
+def test_edge_network_other_kernel_sources(emu, oracle, edge):
+    """k_thermo, k_jacobian and the multi-kernel pipeline (with P and L) on the edge network."""
+    net, atm, okf, okr, want, wp, wl, cols = edge
+    d, keep = descriptor(net)
+    ns, ld, ncol = net.n_species, atm.ld, atm.ncol
+    outs = [np.full((ns, ld), np.nan) for _ in range(4)]
+    assert emu.emu_thermo(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), *[ptr(o) for o in outs], C.c_int(7)) == 0
+    for got, w in zip(outs, oracle.thermo(net, atm.T, ncol)):
+        assert np.all(np.abs(got[:, :ncol] - w[:, :ncol]) <= 1e-12 * (1 + np.abs(w[:, :ncol])))
+    scale = wp + wl
+    for kf_in, kr_in in ((None, None), (okf, okr)):
+        dn, pr, lo = (np.full((ns, ld), np.nan) for _ in range(3))
+        assert emu.emu_source_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                                       ptr(kf_in), ptr(kr_in), ptr(atm.n), ptr(dn), ptr(pr), ptr(lo), C.c_int(16)) == 0
+        G.check_sum(dn, want, scale, cols, "pipeline dn/dt, edge network")
+        G.check_sum(pr, wp, scale, cols, "pipeline P, edge network")
+        G.check_sum(lo, wl, scale, cols, "pipeline L, edge network")
+    h = binding.Network(net, device=-1)
+    rp, col = h.jac_pattern()
+    okf_f, okr_f = okf.copy(), okr.copy()
+    okr_f[~np.isfinite(okr_f)] = 0.0            # the dense oracle wants finite inputs; those columns are not compared
+    wj, sj = oracle.jacobian(net, okf_f, okr_f, atm.n, rp, col, ncol)
+    jac = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf_f), ptr(okr_f), ptr(atm.n), ptr(jac), C.c_int(3)) == 0
+    G.check_sum(jac, wj, sj, cols, "emulated k_jacobian, edge network")
 
 
 TSAN_CHILD = r"""

@@ -3,9 +3,12 @@ evaluated here with numpy exactly as the kernels' formulas read (include/xodiac.
 xod_network_fused_params), must reproduce the oracle's k_f and k_r to the GPU tolerance.  This pins
 the folding of Eq. 7 / 10-12 / 15 and of the per-interval sums of NASA-7
 Gibbs polynomials without a device."""
+import os
+
 import numpy as np
 import pytest
 
+from conftest import ROOT
 from paper_2512_06729_b200 import binding, build
 
 LOG2_KB = np.log2(1.380649e-16)
@@ -89,3 +92,30 @@ def test_large_network_tables_on_sampled_reactions(built, oracle, network):
     fin = np.isfinite(okr) & (np.abs(okr) > 1e-300)
     assert np.all(np.abs(kf - okf) <= 1e-12 * np.abs(okf))
     assert np.all(np.abs(kr[fin] - okr[fin]) <= 1e-12 * np.abs(okr[fin]))
+
+
+def test_exp2_polynomial_constants_match_their_generator():
+    """kExp2C in csrc/xod_math.cuh must be what csrc/gen_exp2_coeffs.py prints (degree 9), and the polynomial
+    must hold the 3.7e-14 relative error the kernel documentation claims (exact rational evaluation)."""
+    import re
+    import subprocess
+    import sys
+    from fractions import Fraction
+    mp = pytest.importorskip("mpmath")
+    csrc = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
+    text = open(os.path.join(csrc, "xod_math.cuh")).read()
+    body = re.search(r"kExp2C\[10\]\s*=\s*\{([^}]*)\}", text).group(1)
+    in_header = [float(x) for x in body.replace("\n", " ").split(",")]
+    out = subprocess.run([sys.executable, os.path.join(csrc, "gen_exp2_coeffs.py"), "9"], capture_output=True, text=True, check=True).stdout
+    generated = {int(m.group(1)): float(m.group(2)) for m in re.finditer(r"c(\d+)\s*=\s*(\S+)", out)}
+    assert in_header == [generated[k] for k in range(10)]
+    mp.mp.dps = 50
+    worst = 0.0
+    for k in range(-400, 401):
+        f = Fraction(k, 800)
+        p = Fraction(0)
+        for c in reversed(in_header):
+            p = p * f + Fraction(c)
+        exact = mp.power(2, mp.mpf(f.numerator) / f.denominator)
+        worst = max(worst, abs(float((mp.mpf(p.numerator) / p.denominator - exact) / exact)))
+    assert worst <= 4e-14
