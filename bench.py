@@ -284,6 +284,12 @@ def stage_timings(binding, h3, net, dev, ws_for, dfma_per_s):
         if big:
             jac = torch.empty((h3.nnz_jac, ld), dtype=torch.float64, device="cuda")
             calls["jacobian"] = lambda: h3.jacobian(ncol, ld, kf, kr, n, jac)
+
+            def jac_gather():
+                h3.tune(binding.XOD_TUNE_JAC_TILED, 0)
+                h3.jacobian(ncol, ld, kf, kr, n, jac)
+                h3.tune(binding.XOD_TUNE_JAC_TILED, 1)
+            calls["jacobian_gather_kernel"] = jac_gather
         res = {"ncol": ncol, "l2": "flushed between calls" if big else "warm (back-to-back calls, as a solver issues them)"}
         for name, fn in calls.items():
             ms = timed(fn, reps, big)

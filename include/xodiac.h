@@ -120,9 +120,14 @@ xod_status xod_network_fused_info(const xod_network *net, int64_t *info);
 xod_status xod_network_fused_params(const xod_network *net, int32_t interval, int32_t *user_rxn, int32_t *kind,
                                     double *coef, double *breakpoints);
 
+/* layout of the tiled Jacobian kernel (xod_jacobian), info[8]: enabled, slots per chunk, chunks, units,
+ * accumulator rows, shared-memory bytes per CTA, distinct derivative slots (k reads per column), padded
+ * schedule entries.  A slot is one distinct d q_{r,dir} / d n_j; the pattern's terms share them. */
+xod_status xod_network_jac_info(const xod_network *net, int64_t *info);
+
 /* host-only consistency check of the internal tables of the fused path (decoded as the kernel
- * decodes them): every source-CSR entry scheduled exactly once, no accumulator row shared by two
- * row tasks of a chunk, species slots intact.  XOD_OK, or XOD_ERR_INVALID_ARG with xod_last_error. */
+ * decodes them): every source-CSR entry and every Jacobian term scheduled exactly once, no
+ * accumulator row shared by two row tasks of a chunk, species slots intact.  XOD_OK, or XOD_ERR_INVALID_ARG with xod_last_error. */
 xod_status xod_network_selfcheck(const xod_network *net);
 
 /* ---- tuning knobs (optional; defaults are chosen for B200) */
@@ -130,7 +135,8 @@ enum {
   XOD_TUNE_CHUNK_COLS = 0, /* columns per pipeline chunk of the fused source call (0 = default) */
   XOD_TUNE_TIMING = 1,     /* != 0: bracket every kernel launch with a CUDA event pair (measurement) */
   XOD_TUNE_SPLIT = 2,      /* reaction splits per column tile of the single-kernel fused path (0 = auto) */
-  XOD_TUNE_FUSED_KERNEL = 3 /* 0: xod_source_fused uses the multi-kernel pipeline instead (default 1) */
+  XOD_TUNE_FUSED_KERNEL = 3, /* 0: xod_source_fused uses the multi-kernel pipeline instead (default 1) */
+  XOD_TUNE_JAC_TILED = 4     /* 0: xod_jacobian uses the one-warp-per-entry gather kernel instead (default 1) */
 };
 xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
 
@@ -139,7 +145,7 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
  * be NULL.  Synchronises on the last recorded event, then clears the record. */
 enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD_KERNEL_RATES_FROM_K = 3,
        XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
-       XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_COUNT = 9 };
+       XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_JAC_TILED = 9, XOD_KERNEL_COUNT = 10 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);

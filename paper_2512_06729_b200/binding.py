@@ -16,8 +16,8 @@ _lib = None
 XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK = 1
-XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL = 0, 1, 2, 3
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs"]
+XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL, XOD_TUNE_JAC_TILED = 0, 1, 2, 3, 4
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -27,7 +27,7 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
            "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params",
-           "xod_check_status", "xod_build_has_checks"]
+           "xod_check_status", "xod_build_has_checks", "xod_network_jac_info"]
 
 
 class XodError(RuntimeError):
@@ -153,6 +153,12 @@ class Network:
         v = (C.c_int64 * 10)()
         _check(lib().xod_network_fused_info(self._h, v))
         keys = ("enabled", "chunk", "nchunk", "n_acc", "n_bp", "smem_bytes", "npad", "tasks", "entries", "rev_bytes")
+        return dict(zip(keys, [int(x) for x in v]))
+
+    def jac_info(self):
+        v = (C.c_int64 * 8)()
+        _check(lib().xod_network_jac_info(self._h, v))
+        keys = ("enabled", "chunk", "nchunk", "units", "acc_rows", "smem_bytes", "slots", "entries")
         return dict(zip(keys, [int(x) for x in v]))
 
     def fused_params(self, interval):

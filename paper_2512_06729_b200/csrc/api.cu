@@ -8,6 +8,7 @@
 #include <string>
 
 #include "fused.cuh"
+#include "jac_tiled.cuh"
 #include "rates2.cuh"
 #include "kernels.cuh"
 
@@ -174,6 +175,15 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (net->h.f.enabled && fused_smem_bytes(net->h.ns, net->h.f.n_acc, chunk, net->h.f.meta_cap) <= kFusedSmemMax) break;
       net->h.f.enabled = false;
     }
+    // tables of the tiled Jacobian kernel: the largest chunk whose shared memory fits one CTA
+    for (int chunk : {4 * kFPass, 3 * kFPass, 2 * kFPass, kFPass}) {
+      const int64_t fixed = ((int64_t)(net->h.ns + 1) + 2 * (chunk + 1)) * kFW * 8 + 2 * 12 * 1024;  // schedules: guess, checked below
+      const int64_t budget = ((int64_t)kFusedSmemMax - fixed) / (kFW * 8);
+      if (budget < 1) continue;
+      pack_jac_tiled(net->h, chunk, (int)std::min<int64_t>(budget, 0xfff0));
+      if (net->h.jt.enabled && jac_tiled_smem_bytes(net->h.ns, net->h.jt.acc_rows, chunk, net->h.jt.meta_cap) <= kFusedSmemMax) break;
+      net->h.jt.enabled = false;
+    }
   } catch (const std::bad_alloc &) {
     delete net;
     return fail(XOD_ERR_ALLOC, "out of host memory while packing");
@@ -223,9 +233,28 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
           ce = cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
         if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_fused)");
       }
+    }
+    {
       int smc = 0;
       if (cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, cuda_device) == cudaSuccess && smc > 0)
         net->sm_count = smc;
+    }
+    if (h.jt.enabled) {
+      JacTiledHost &t = h.jt;
+      JacTiledDev &jd = net->jd;
+      jd.enabled = 1;
+      jd.chunk = t.chunk, jd.nchunk = t.nchunk, jd.acc_rows = t.acc_rows, jd.meta_cap = t.meta_cap;
+      jd.n_flush = (int32_t)(t.flush.size() / 4);
+      const int32_t *p4 = nullptr;
+      if (st == XOD_OK) st = upload(net, t.meta_ptr, &jd.meta_ptr);
+      if (st == XOD_OK) st = upload(net, t.meta, &p4), jd.meta = reinterpret_cast<const int4 *>(p4);
+      if (st == XOD_OK) st = upload(net, t.slots, &p4), jd.slots = reinterpret_cast<const int4 *>(p4);
+      if (st == XOD_OK) st = upload(net, t.chunk_info, &p4), jd.chunk_info = reinterpret_cast<const int4 *>(p4);
+      if (st == XOD_OK) st = upload(net, t.flush, &p4), jd.flush = reinterpret_cast<const int4 *>(p4);
+      if (st == XOD_OK) {
+        cudaError_t ce = cudaFuncSetAttribute(k_jac_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
+        if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_jac_tiled)");
+      }
     }
 #undef UP
     if (st != XOD_OK) {
@@ -327,10 +356,20 @@ xod_status xod_network_fused_params(const xod_network *net, int32_t interval, in
   return XOD_OK;
 }
 
+xod_status xod_network_jac_info(const xod_network *net, int64_t *info) {
+  if (!net || !info) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
+  const JacTiledHost &t = net->h.jt;
+  info[0] = t.enabled, info[1] = t.chunk, info[2] = t.nchunk, info[3] = t.n_units, info[4] = t.acc_rows;
+  info[5] = t.enabled ? (int64_t)jac_tiled_smem_bytes(net->h.ns, t.acc_rows, t.chunk, t.meta_cap) : 0;
+  info[6] = t.n_slots, info[7] = t.n_entries;
+  return XOD_OK;
+}
+
 xod_status xod_network_selfcheck(const xod_network *net) {
   if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
   std::string err;
   if (!check_fused(net->h, err)) return fail(XOD_ERR_INVALID_ARG, err);
+  if (!check_jac_tiled(net->h, err)) return fail(XOD_ERR_INVALID_ARG, err);
   return XOD_OK;
 }
 
@@ -348,6 +387,10 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value) {
   }
   if (knob == XOD_TUNE_FUSED_KERNEL) {
     net->use_fused = value;
+    return XOD_OK;
+  }
+  if (knob == XOD_TUNE_JAC_TILED) {
+    net->use_jac_tiled = value;
     return XOD_OK;
   }
   if (knob == XOD_TUNE_TIMING) {
@@ -619,6 +662,30 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
   if (!n || !jac) return fail(XOD_ERR_INVALID_ARG, "n or jac is NULL");
   if (net->h.nr > 0 && (!kf || !kr)) return fail(XOD_ERR_INVALID_ARG, "kf or kr is NULL");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (net->jd.enabled && net->use_jac_tiled && net->h.nr > 0) {
+    // whole rounds of column tiles on every SM run unsplit; the last partial round (or a batch with fewer
+    // tiles than SMs) has each tile's units split over the otherwise idle SMs (units are independent)
+    const size_t smem = jac_tiled_smem_bytes(net->h.ns, net->h.jt.acc_rows, net->h.jt.chunk, net->h.jt.meta_cap);
+    const int64_t ntiles = (ncol + kFW - 1) / kFW, sm = net->sm_count;
+    const int64_t full = net->force_split > 0 ? 0 : ntiles / sm * sm;
+    for (int part = 0; part < 2; ++part) {
+      const int64_t t0 = part == 0 ? 0 : full, t1 = part == 0 ? full : ntiles;
+      if (t1 <= t0) continue;
+      JacArgs a{};
+      const int64_t c0 = t0 * kFW;
+      a.ncol = std::min<int64_t>(ncol, t1 * kFW) - c0, a.ld = ld;
+      a.kf = kf + c0, a.kr = kr + c0, a.n = n + c0, a.jac = jac + c0;
+      a.ntiles = (int32_t)(t1 - t0);
+      int64_t split = part == 0 ? 1 : (net->force_split > 0 ? net->force_split : sm / (t1 - t0));
+      a.nsplit = (int32_t)std::max<int64_t>(1, std::min<int64_t>(split, net->h.jt.n_units));
+      a.nr = net->h.nr, a.nnz = net->d.nnz_jac;
+      const unsigned grid = (unsigned)std::min<int64_t>((int64_t)a.ntiles * a.nsplit, sm);
+      Timed tm(net, KID_JAC_TILED, s);
+      k_jac_tiled<<<grid, kFWarps * 32, smem, s>>>(net->jd, net->h.ns, a);
+      XOD_CUDA(cudaGetLastError());
+    }
+    return XOD_OK;
+  }
   const int64_t ncg = (ncol + 31) / 32;
   if (ncg > 65535) return fail(XOD_ERR_INVALID_ARG, "ncol too large for one xod_jacobian call (max 2097120)");
   const int64_t want = (net->d.nnz_jac + 7) / 8;

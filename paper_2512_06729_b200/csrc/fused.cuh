@@ -28,6 +28,7 @@
 #include "xod_internal.h"
 #include "xod_math.cuh"
 #include <xod_cta.cuh>  // CTA primitives (dynamic shared memory, cp.async); resolved through -I csrc
+#include "sched.cuh"
 
 namespace xod {
 
@@ -42,7 +43,6 @@ struct FusedArgs {
   double log2_kb;
 };
 
-__device__ __forceinline__ double2 lds2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
 __device__ __forceinline__ double2 ldg2(const unsigned char *p) { return __ldg(reinterpret_cast<const double2 *>(p)); }
 
 // log2 k_r (UNI/BI) or z (FALLOFF) from the block of interval g
@@ -202,72 +202,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       cp_async_wait_all();
       __syncthreads();
       // ------------------------------------------------------------ phase B
-      const int *hdr = reinterpret_cast<const int *>(mb);
-      const int t_begin = hdr[warp], t_end = XOD_IDX(hdr[warp + 1], f.meta_cap - kFMetaHdr / 4 + 1);
-      const unsigned *ent = reinterpret_cast<const unsigned *>(mb + kFMetaHdr / 4 + XOD_IDX(hdr[kFWarps + 1], f.meta_cap - kFMetaHdr / 4 + 1)) + grp;
-      const int ent_words = (f.meta_cap - kFMetaHdr / 4 - hdr[kFWarps + 1]) * 4;  // XOD_CHECK: words of the entry section
-      (void)ent_words;
-      const double *q_l = qb + l2;
-      // two warp tasks in flight per iteration (their loads are independent): the dependent
-      // chain header -> entry -> q -> FMA is the latency that matters here, not the instruction count
-      auto row_of = [&](const int4 &tk) {
-        const unsigned rows = (grp & 2) ? (unsigned)tk.w : (unsigned)tk.z;
-        return (int)((grp & 1) ? rows >> 16 : rows & 0xffffu);
-      };
-      auto add_row = [&](int row, double s0, double s1) {
-        if (row != 0xffff) {
-          double2 *dst = reinterpret_cast<double2 *>(acc_s + (size_t)XOD_IDX(row, f.n_acc) * kFW + l2);
-          double2 cur = *dst;
-          cur.x += s0, cur.y += s1;
-          *dst = cur;
-        }
-      };
-      int t = t_begin;
-#pragma unroll 1
-      for (; t + 1 < t_end; t += 2) {
-        const int4 ta = mb[kFMetaHdr / 4 + t], tb = mb[kFMetaHdr / 4 + t + 1];
-        const unsigned *ea = ent + ta.x, *eb = ent + tb.x;
-        double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
-        const int nmin = min(ta.y, tb.y);
-        int st = 0;
-#pragma unroll 1
-        for (; st < nmin; ++st) {
-          const unsigned xa = ea[XOD_IDX(ta.x + st * 4 + grp, ent_words) - ta.x - grp], xb = eb[XOD_IDX(tb.x + st * 4 + grp, ent_words) - tb.x - grp];
-          const double2 qa = lds2(q_l + XOD_IDX(xa & 0xffffu, qrows) * kFW), qc = lds2(q_l + XOD_IDX(xb & 0xffffu, qrows) * kFW);
-          const double na = __hiloint2double((int)(xa & 0xffff0000u), 0), nb = __hiloint2double((int)(xb & 0xffff0000u), 0);
-          a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
-          b0 = fma(nb, qc.x, b0), b1 = fma(nb, qc.y, b1);
-        }
-#pragma unroll 1
-        for (int s2 = st; s2 < ta.y; ++s2) {
-          const unsigned xa = ea[XOD_IDX(ta.x + s2 * 4 + grp, ent_words) - ta.x - grp];
-          const double2 qa = lds2(q_l + XOD_IDX(xa & 0xffffu, qrows) * kFW);
-          const double na = __hiloint2double((int)(xa & 0xffff0000u), 0);
-          a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
-        }
-#pragma unroll 1
-        for (int s2 = st; s2 < tb.y; ++s2) {
-          const unsigned xb = eb[XOD_IDX(tb.x + s2 * 4 + grp, ent_words) - tb.x - grp];
-          const double2 qc = lds2(q_l + XOD_IDX(xb & 0xffffu, qrows) * kFW);
-          const double nb = __hiloint2double((int)(xb & 0xffff0000u), 0);
-          b0 = fma(nb, qc.x, b0), b1 = fma(nb, qc.y, b1);
-        }
-        add_row(row_of(ta), a0, a1);
-        add_row(row_of(tb), b0, b1);
-      }
-      if (t < t_end) {
-        const int4 ta = mb[kFMetaHdr / 4 + t];
-        const unsigned *ea = ent + ta.x;
-        double a0 = 0.0, a1 = 0.0;
-#pragma unroll 1
-        for (int st = 0; st < ta.y; ++st) {
-          const unsigned xa = ea[XOD_IDX(ta.x + st * 4 + grp, ent_words) - ta.x - grp];
-          const double2 qa = lds2(q_l + XOD_IDX(xa & 0xffffu, qrows) * kFW);
-          const double na = __hiloint2double((int)(xa & 0xffff0000u), 0);
-          a0 = fma(na, qa.x, a0), a1 = fma(na, qa.y, a1);
-        }
-        add_row(row_of(ta), a0, a1);
-      }
+      sched_reduce(mb, qb, acc_s, warp, grp, l2, qrows, f.n_acc, f.meta_cap);
     }
     __syncthreads();
     // ---- extra rows of hub species -> their species row, in row order (fixed order)

@@ -46,6 +46,49 @@ size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap) {
          2 * (size_t)meta_cap * 16 + (size_t)kFW * (4 * sizeof(double) + sizeof(int32_t));
 }
 
+// The production/loss schedule of one chunk (shared by k_fused and k_jac_tiled): row tasks (an
+// accumulator row and <= kFSegMax entries) are sorted by length, four similar-length ones form a
+// warp task whose entries are interleaved [step][lane group], and warp tasks are dealt to the
+// least-loaded warp, longest first.  blob = header (kFWarps + 1 task offsets, task count, two
+// spare words) | tasks | entries, in 16-byte units.
+void build_chunk_schedule(std::vector<SchedSeg> segs, uint32_t zero_entry, std::vector<int32_t> &blob,
+                          int64_t &n_tasks, int64_t &n_entries) {
+  std::stable_sort(segs.begin(), segs.end(), [](const SchedSeg &a, const SchedSeg &b) { return a.len > b.len; });
+  std::vector<std::vector<FusedTask>> per_warp(kFWarps);
+  std::vector<int> load(kFWarps, 0);
+  std::vector<uint32_t> entries;
+  for (size_t s0 = 0; s0 < segs.size(); s0 += 4) {
+    const int cnt = (int)std::min<size_t>(4, segs.size() - s0), nsteps = segs[s0].len;
+    FusedTask t;
+    t.entry_off = (int32_t)entries.size();
+    t.nsteps = nsteps;
+    uint32_t r[4] = {0xffffu, 0xffffu, 0xffffu, 0xffffu};
+    for (int g = 0; g < cnt; ++g) r[g] = (uint32_t)segs[s0 + g].row;
+    t.rows01 = (int32_t)(r[0] | (r[1] << 16));
+    t.rows23 = (int32_t)(r[2] | (r[3] << 16));
+    for (int st = 0; st < nsteps; ++st)
+      for (int g = 0; g < 4; ++g)
+        entries.push_back(g < cnt && st < segs[s0 + g].len ? segs[s0 + g].ent[st] : zero_entry);
+    const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+    load[w] += nsteps + 2;
+    per_warp[w].push_back(t);
+  }
+  blob.assign(kFMetaHdr, 0);
+  int nt = 0;
+  for (int w = 0; w < kFWarps; ++w) {
+    blob[w] = nt;
+    nt += (int)per_warp[w].size();
+  }
+  blob[kFWarps] = nt, blob[kFWarps + 1] = nt;
+  for (int w = 0; w < kFWarps; ++w)
+    for (const FusedTask &t : per_warp[w]) {
+      blob.push_back(t.entry_off), blob.push_back(t.nsteps), blob.push_back(t.rows01), blob.push_back(t.rows23);
+    }
+  for (uint32_t e : entries) blob.push_back((int32_t)e);
+  while (blob.size() % 4) blob.push_back((int32_t)zero_entry);
+  n_tasks = nt, n_entries = (int64_t)entries.size();
+}
+
 void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
   FusedHost &f = h.f;
   f = FusedHost();
@@ -185,13 +228,12 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
     }
   if (f.n_acc >= 0xffff) return;
 
-  struct Seg { int32_t row; const uint32_t *ent; int len; };
   const uint32_t zero_entry = (uint32_t)chunk;  // nu bits 0 (= +0.0), the zero row of q
   f.meta_ptr.assign((size_t)nchunk + 1, 0);
   f.meta.clear();
   f.meta_cap = 0, f.n_tasks = 0, f.n_entries = 0;
   for (int k = 0; k < nchunk; ++k) {
-    std::vector<Seg> segs;
+    std::vector<SchedSeg> segs;
     for (const Row &r : rows[k]) {
       const int len = (int)r.ent.size(), nseg = (len + kFSegMax - 1) / kFSegMax, per = (len + nseg - 1) / nseg;
       for (int s = 0; s < nseg; ++s) {
@@ -199,45 +241,13 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
         if (e > b) segs.push_back({s == 0 ? r.species : extra_base[r.species] + s - 1, r.ent.data() + b, e - b});
       }
     }
-    std::stable_sort(segs.begin(), segs.end(), [](const Seg &a, const Seg &b) { return a.len > b.len; });
-    // warp tasks of 4 similar-length segments, dealt to the least-loaded warp (longest first)
-    std::vector<std::vector<FusedTask>> per_warp(kFWarps);
-    std::vector<int> load(kFWarps, 0);
-    std::vector<uint32_t> entries;
-    for (size_t s0 = 0; s0 < segs.size(); s0 += 4) {
-      const int cnt = (int)std::min<size_t>(4, segs.size() - s0), nsteps = segs[s0].len;
-      FusedTask t;
-      t.entry_off = (int32_t)entries.size();
-      t.nsteps = nsteps;
-      uint32_t r[4] = {0xffffu, 0xffffu, 0xffffu, 0xffffu};
-      for (int g = 0; g < cnt; ++g) r[g] = (uint32_t)segs[s0 + g].row;
-      t.rows01 = (int32_t)(r[0] | (r[1] << 16));
-      t.rows23 = (int32_t)(r[2] | (r[3] << 16));
-      for (int st = 0; st < nsteps; ++st)
-        for (int g = 0; g < 4; ++g)
-          entries.push_back(g < cnt && st < segs[s0 + g].len ? segs[s0 + g].ent[st] : zero_entry);
-      const int w = (int)(std::min_element(load.begin(), load.end()) - load.begin());
-      load[w] += nsteps + 2;
-      per_warp[w].push_back(t);
-    }
-    // blob: header (17 task offsets per warp, task count) | tasks | entries, 16-byte units
-    std::vector<int32_t> blob(kFMetaHdr, 0);
-    int nt = 0;
-    for (int w = 0; w < kFWarps; ++w) {
-      blob[w] = nt;
-      nt += (int)per_warp[w].size();
-    }
-    blob[kFWarps] = nt, blob[kFWarps + 1] = nt;
-    for (int w = 0; w < kFWarps; ++w)
-      for (const FusedTask &t : per_warp[w]) {
-        blob.push_back(t.entry_off), blob.push_back(t.nsteps), blob.push_back(t.rows01), blob.push_back(t.rows23);
-      }
-    for (uint32_t e : entries) blob.push_back((int32_t)e);
-    while (blob.size() % 4) blob.push_back((int32_t)zero_entry);
+    std::vector<int32_t> blob;
+    int64_t nt = 0, nent = 0;
+    build_chunk_schedule(segs, zero_entry, blob, nt, nent);
+    f.n_tasks += nt, f.n_entries += nent;
     f.meta.insert(f.meta.end(), blob.begin(), blob.end());
     f.meta_ptr[k + 1] = (int32_t)(f.meta.size() / 4);
     f.meta_cap = std::max<int32_t>(f.meta_cap, (int32_t)(blob.size() / 4));
-    f.n_tasks += nt, f.n_entries += (int64_t)entries.size();
   }
   f.enabled = true;
 }

@@ -114,6 +114,29 @@ struct FusedHost {
   std::vector<int32_t> meta;           // 4 words per 16-byte unit
 };
 
+// ---- tables of the tiled Jacobian kernel (k_jac_tiled, jac_tiled.cuh; packed by pack_jac.cpp) ----
+// A *slot* is one distinct derivative d q_{r,dir} / d n_j = m k[dir][r] n[o1] n[o2]; all terms of the
+// entries (i, j) of one Jacobian column j draw on the slots of that column only.  Columns are grouped
+// into *units* (several small columns, or one hub column); a unit is processed in chunks of `chunk`
+// slots; its entries own accumulator rows that are flushed to jac[e][col] when the unit ends.
+struct JacTiledHost {
+  bool enabled = false;
+  int32_t chunk = 0, nchunk = 0, n_units = 0, acc_rows = 0, meta_cap = 0;
+  int64_t n_slots = 0, n_tasks = 0, n_entries = 0;
+  std::vector<int32_t> meta_ptr;    // [nchunk + 1] in 16-byte units into meta
+  std::vector<int32_t> meta;        // per chunk: header | tasks | entries (build_chunk_schedule)
+  std::vector<int32_t> slots;       // [nchunk * chunk][4]: rk (user reaction, bit 31 = reverse), o1, o2 (ns = none), 0
+  std::vector<int32_t> chunk_info;  // [nchunk][4]: first chunk of the unit, flush begin, flush end (last chunk of a unit only), slots used
+  std::vector<int32_t> flush;       // [n_flush][4]: pattern entry e, first accumulator row, rows, 0
+};
+
+struct JacTiledDev {
+  int32_t enabled;
+  int32_t chunk, nchunk, acc_rows, meta_cap, n_flush;
+  const int32_t *meta_ptr;
+  const int4 *meta, *slots, *chunk_info, *flush;
+};
+
 struct HostTables {
   int32_t ns = 0, ne = 0, nr = 0, n_photo = 0;
   int32_t uni_begin = 0, bi_begin = 0, fo_begin = 0, ph_begin = 0;
@@ -133,7 +156,13 @@ struct HostTables {
   std::vector<int64_t> jac_term_ptr;
   std::vector<JacTerm> jac_terms;
   FusedHost f;
+  JacTiledHost jt;
 };
+
+// one row task of a chunk schedule: an accumulator row and its entries (q row | nu bits)
+struct SchedSeg { int32_t row; const uint32_t *ent; int len; };
+void build_chunk_schedule(std::vector<SchedSeg> segs, uint32_t zero_entry, std::vector<int32_t> &blob,
+                          int64_t &n_tasks, int64_t &n_entries);
 
 // pack.cpp
 xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &err);
@@ -143,13 +172,17 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk);
 bool check_fused(const HostTables &h, std::string &err);
 // shared-memory bytes k_fused needs for these tables
 size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap);
+// pack_jac.cpp: tables of the tiled Jacobian kernel for a given chunk size and accumulator-row budget
+void pack_jac_tiled(HostTables &h, int chunk, int acc_budget);
+bool check_jac_tiled(const HostTables &h, std::string &err);
+size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 
 }  // namespace xod
 
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused
@@ -164,8 +197,10 @@ struct xod_network {
   xod::HostTables h;
   xod::DevTables d{};
   xod::FusedDev fd{};
+  xod::JacTiledDev jd{};
   int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
   int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
+  int64_t use_jac_tiled = 1;  // XOD_TUNE_JAC_TILED: 0 = the one-warp-per-entry gather kernel
   int sm_count = 148;       // replaced by the device attribute at create
   int device = -1;
   std::vector<void *> dev_allocs;

@@ -17,6 +17,7 @@ void emu_syncthreads() { g_barrier->arrive_and_wait(); }
 
 #include "../../paper_2512_06729_b200/csrc/fused.cuh"
 #include "../../paper_2512_06729_b200/csrc/rates2.cuh"
+#include "../../paper_2512_06729_b200/csrc/jac_tiled.cuh"
 #include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
@@ -157,6 +158,40 @@ int emu_jacobian(const xod_network_desc *desc, int64_t ncol, int64_t ld, const d
   if (pack_network(desc, h, err) != XOD_OK) return 1;
   const DevTables d = dev_tables(h);
   run_grid((unsigned)gx, (unsigned)((ncol + 31) / 32), 256, false, [&] { k_jacobian(d, ncol, ld, kf, kr, n, jac); });
+  return 0;
+}
+
+// Jacobian values by k_jac_tiled on `grid` blocks, each tile's units split over `nsplit` work items
+int emu_jacobian_tiled(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                       const double *n, double *jac, int grid, int nsplit) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK || ncol <= 0) return 1;
+  for (int chunk : {4 * kFPass, 3 * kFPass, 2 * kFPass, kFPass}) {
+    const int64_t fixed = ((int64_t)(h.ns + 1) + 2 * (chunk + 1)) * kFW * 8 + 2 * 12 * 1024;
+    const int64_t budget = ((int64_t)kSmemMax - fixed) / (kFW * 8);
+    if (budget < 1) continue;
+    pack_jac_tiled(h, chunk, (int)std::min<int64_t>(budget, 0xfff0));
+    if (h.jt.enabled && jac_tiled_smem_bytes(h.ns, h.jt.acc_rows, chunk, h.jt.meta_cap) <= kSmemMax) break;
+    h.jt.enabled = false;
+  }
+  if (!h.jt.enabled || !check_jac_tiled(h, err)) return 2;
+  const JacTiledHost &t = h.jt;
+  JacTiledDev jd{};
+  jd.enabled = 1, jd.chunk = t.chunk, jd.nchunk = t.nchunk, jd.acc_rows = t.acc_rows, jd.meta_cap = t.meta_cap;
+  jd.n_flush = (int32_t)(t.flush.size() / 4);
+  jd.meta_ptr = t.meta_ptr.data();
+  jd.meta = reinterpret_cast<const int4 *>(t.meta.data());
+  jd.slots = reinterpret_cast<const int4 *>(t.slots.data());
+  jd.chunk_info = reinterpret_cast<const int4 *>(t.chunk_info.data());
+  jd.flush = reinterpret_cast<const int4 *>(t.flush.data());
+  JacArgs a{};
+  a.ncol = ncol, a.ld = ld, a.kf = kf, a.kr = kr, a.n = n, a.jac = jac;
+  a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
+  a.nsplit = std::max(1, std::min(nsplit, (int)t.n_units));
+  a.nr = h.nr, a.nnz = (int64_t)h.jac_col.size();
+  const int ns = h.ns;
+  run_grid((unsigned)grid, 1, kFWarps * 32, true, [&] { k_jac_tiled(jd, ns, a); });
   return 0;
 }
 

@@ -244,11 +244,15 @@ def test_jacobian_matches_oracle(xod, oracle, network, cfg, n_atm):
     okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
     rp, col = h.jac_pattern()
     want, scale = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
-    jac = G.empty(h.nnz_jac, atm.ld)
-    h.jacobian(ncol, atm.ld, G.dev(okf), G.dev(okr), G.dev(atm.n), jac)
-    got = G.host(jac)
-    G.check_sum(got, want, scale, np.arange(ncol), "Jacobian config %d" % cfg)
-    assert np.all(np.isnan(got[:, ncol:]))
+    assert h.jac_info()["enabled"] == 1
+    for tiled in (0, 1):      # the one-warp-per-entry gather kernel, then the tiled kernel (the default)
+        h.tune(xod.XOD_TUNE_JAC_TILED, tiled)
+        jac = G.empty(h.nnz_jac, atm.ld)
+        h.jacobian(ncol, atm.ld, G.dev(okf), G.dev(okr), G.dev(atm.n), jac)
+        got = G.host(jac)
+        worst = G.check_sum(got, want, scale, np.arange(ncol), "Jacobian config %d (tiled %d)" % (cfg, tiled))
+        assert np.all(np.isnan(got[:, ncol:]))
+        print("Jacobian config %d, %d columns, tiled kernel %d: worst |err|/scale %.2e" % (cfg, ncol, tiled, worst))
     # element conservation of the Jacobian: sum_i a_ie Jac_ij = 0 for every (e, j)
     rows = np.repeat(np.arange(net.n_species), np.diff(rp))
     a = net.composition.astype(np.float64)
@@ -553,10 +557,16 @@ def test_edge_network_jacobian_and_thermo(xod, oracle, edge):
     okr_f = np.where(np.isfinite(okr), okr, 0.0)      # finite inputs for the dense oracle; those columns are not compared
     rp, col = h.jac_pattern()
     wj, sj = oracle.jacobian(net, okf, okr_f, atm.n, rp, col, ncol)
-    jac = G.empty(h.nnz_jac, ld)
-    h.jacobian(ncol, ld, G.dev(okf), G.dev(okr_f), G.dev(atm.n), jac)
-    worst = G.check_sum(G.host(jac), wj, sj, cols, "edge Jacobian")
-    print("edge network Jacobian: worst |err|/scale %.2e" % worst)
+    for tiled in (0, 1):
+        h.tune(xod.XOD_TUNE_JAC_TILED, tiled)
+        for split in (0, 3):
+            h.tune(xod.XOD_TUNE_SPLIT, split)
+            jac = G.empty(h.nnz_jac, ld)
+            h.jacobian(ncol, ld, G.dev(okf), G.dev(okr_f), G.dev(atm.n), jac)
+            worst = G.check_sum(G.host(jac), wj, sj, cols, "edge Jacobian (tiled %d, split %d)" % (tiled, split))
+            assert np.all(np.isnan(G.host(jac)[:, ncol:]))
+            print("edge network Jacobian (tiled %d, split %d): worst |err|/scale %.2e" % (tiled, split, worst))
+    h.tune(xod.XOD_TUNE_SPLIT, 0)
     outs = [G.empty(net.n_species, ld) for _ in range(4)]
     h.thermo(ncol, ld, G.dev(atm.T), *outs)
     for got, w, s in zip(outs, oracle.thermo(net, atm.T, ncol), thermo_scale(net, atm.T)):

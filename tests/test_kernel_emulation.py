@@ -18,8 +18,8 @@ from paper_2512_06729_b200 import binding
 EMU_DIR = os.path.join(ROOT, "tests", "kernel_emu")
 CSRC = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
 LIB = os.path.join(EMU_DIR, "libxod_emu.so")
-SOURCES = [os.path.join(EMU_DIR, "emu.cpp"), os.path.join(CSRC, "pack.cpp"), os.path.join(CSRC, "pack_fused.cpp")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "xod_math.cuh", "xod_internal.h")] + [
+SOURCES = [os.path.join(EMU_DIR, "emu.cpp")] + [os.path.join(CSRC, f) for f in ("pack.cpp", "pack_fused.cpp", "pack_jac.cpp")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "jac_tiled.cuh", "sched.cuh", "xod_math.cuh", "xod_internal.h")] + [
     os.path.join(EMU_DIR, "shim", "cuda_runtime.h"), os.path.join(EMU_DIR, "shim", "xod_cta.cuh")]
 
 
@@ -135,6 +135,50 @@ def test_thermo_and_jacobian_kernel_sources_match_oracle(emu, oracle, network, c
     assert emu.emu_jacobian(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr), ptr(atm.n), ptr(jac), C.c_int(3)) == 0
     assert np.all(np.abs(jac[:, :ncol] - wj[:, :ncol]) <= 1e-11 * sj[:, :ncol])
     assert np.all(np.isnan(jac[:, ncol:]))
+
+
+@pytest.mark.parametrize("cfg,grid,nsplit", [(1, 1, 1), (2, 2, 1), (2, 3, 3), (2, 30, 5)])
+def test_tiled_jacobian_kernel_source_matches_oracle(emu, oracle, network, cfg, grid, nsplit):
+    """k_jac_tiled: slots evaluated once per column tile, scheduled row reduction, per-unit flush; fewer blocks
+    than work items (persistent loop) and the units of a tile split over several blocks."""
+    from paper_2512_06729_b200 import synth
+    net = network(cfg)
+    atm = synth.config_atmosphere(cfg, net)
+    d, keep = descriptor(net)
+    ncol, ld = atm.ncol, atm.ld
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    h = binding.Network(net, device=-1)
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
+    jac = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr), ptr(atm.n), ptr(jac),
+                                  C.c_int(grid), C.c_int(nsplit)) == 0
+    worst = G.check_sum(jac, wj, sj, np.arange(ncol), "emulated k_jac_tiled config %d" % cfg)
+    assert np.all(np.isnan(jac[:, ncol:])), "padding columns written"
+    print("k_jac_tiled config %d (grid %d, split %d): worst |err|/scale %.2e" % (cfg, grid, nsplit, worst))
+
+
+def test_tiled_jacobian_kernel_source_hub_columns_over_several_chunks(emu, oracle, network):
+    """Config-3 network: hub species own units of several chunks (accumulators carried across chunks, extra rows
+    for entries with more than 16 terms in a chunk); 20 columns = one full and one ragged tile, units split 3 ways."""
+    from paper_2512_06729_b200 import synth
+    net = network(3)
+    atm = synth.make_atmosphere(2033, net, 1, 20)
+    d, keep = descriptor(net)
+    ncol, ld = atm.ncol, atm.ld
+    h = binding.Network(net, device=-1)
+    info = h.jac_info()
+    assert info["enabled"] and info["nchunk"] > info["units"], "some unit must span several chunks"
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
+    jac = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr), ptr(atm.n), ptr(jac),
+                                  C.c_int(2), C.c_int(3)) == 0
+    worst = G.check_sum(jac, wj, sj, np.arange(ncol), "emulated k_jac_tiled config 3")
+    assert np.all(np.isnan(jac[:, ncol:]))
+    print("k_jac_tiled config 3 (%d slots for %d terms, %d chunks, %d units): worst |err|/scale %.2e"
+          % (info["slots"], h.n_jac_terms, info["nchunk"], info["units"], worst))
 
 
 @pytest.mark.parametrize("cfg", [1, 2])
@@ -261,6 +305,11 @@ def test_edge_network_other_kernel_sources(emu, oracle, edge):
     jac = np.full((col.shape[0], ld), np.nan)
     assert emu.emu_jacobian(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf_f), ptr(okr_f), ptr(atm.n), ptr(jac), C.c_int(3)) == 0
     G.check_sum(jac, wj, sj, cols, "emulated k_jacobian, edge network")
+    jac2 = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf_f), ptr(okr_f), ptr(atm.n), ptr(jac2),
+                                  C.c_int(2), C.c_int(2)) == 0
+    G.check_sum(jac2, wj, sj, cols, "emulated k_jac_tiled, edge network")
+    assert np.all(np.isnan(jac2[:, ncol:]))
 
 
 TSAN_CHILD = r"""
@@ -269,21 +318,31 @@ sys.path.insert(0, sys.argv[1]); sys.path.insert(0, sys.argv[1] + "/tests")
 import numpy as np
 import test_kernel_emulation as tk
 from paper_2512_06729_b200 import synth
+from paper_2512_06729_b200 import binding
+def binding_nnz(net):
+    return binding.Network(net, device=-1).nnz_jac
 emu = C.CDLL(sys.argv[2])
 net = synth.config_network(2)
 atm = synth.config_atmosphere(2, net)
 for grid, nsplit in ((3, 1), (5, 3)):
     got = tk.run_fused(emu, net, atm, atm.ncol, grid=grid, nsplit=nsplit)
     assert np.all(np.isfinite(got[:, :atm.ncol]))
+# the tiled Jacobian kernel: slot buffers, accumulator rows flushed and zeroed per unit
+d, keep = tk.descriptor(net)
+ncol = 40
+kf = np.abs(np.random.default_rng(1).normal(size=(net.n_reactions, atm.ld)))
+jac = np.zeros((binding_nnz(net), atm.ld))
+assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(atm.ld), tk.ptr(kf), tk.ptr(kf), tk.ptr(atm.n),
+                              tk.ptr(jac), C.c_int(2), C.c_int(2)) == 0
 print("emulated-ok")
 """
 
 
-def test_fused_kernel_source_is_race_free_under_thread_sanitizer():
+def test_fused_and_tiled_jacobian_kernel_sources_are_race_free_under_thread_sanitizer():
     """racecheck substitute (compute-sanitizer is closed on the GPU pool): the emulated CUDA threads are
     real threads and __syncthreads a real barrier, so ThreadSanitizer sees every shared-memory access
-    of k_fused between barriers: the double-buffered q and schedule, the accumulator read-modify-writes
-    of the row tasks, the tile prologue/epilogue.  (Removing the per-chunk barrier makes it report.)"""
+    of k_fused and k_jac_tiled between barriers: the double-buffered values and schedule, the accumulator
+    read-modify-writes of the row tasks, the per-unit flush, the tile prologue/epilogue.  (Removing the per-chunk barrier makes it report.)"""
     tsan = subprocess.run(["gcc", "-print-file-name=libtsan.so"], capture_output=True, text=True).stdout.strip()
     if not os.path.isabs(tsan) or not os.path.exists(tsan):
         pytest.skip("libtsan not available")
