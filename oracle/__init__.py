@@ -174,3 +174,28 @@ class Oracle:
         if bad != 0:
             raise AssertionError("oracle: %d dense Jacobian entries outside the pattern are non-zero" % bad)
         return jac, sc
+
+    # ---- f1: backward-Euler Newton step
+    def newton_system(self, net, kf, kr, n_old, dt, y, c):
+        """A = I - dt Jac(y) [ns][ns] and b = -(y - n_old - dt f(y)) [ns] of column c, rounded to double."""
+        kf, kr, n_old, y, dt = _f64(kf), _f64(kr), _f64(n_old), _f64(y), _f64(dt)
+        ns, _ = self._dims(net)
+        s, keep = self._net(net)
+        A, b = np.zeros((ns, ns)), np.zeros(ns)
+        rc = self.lib.orc_newton_system(C.byref(s), C.c_long(y.shape[1]), _ptr(kf), _ptr(kr), _ptr(n_old), _ptr(dt),
+                                        _ptr(y), C.c_long(c), _ptr(A), _ptr(b))
+        assert rc == 0
+        return A, b
+
+    def newton_step(self, net, kf, kr, n_old, dt, y, ncol=None):
+        """delta, y + delta [n_species][ld] of one Newton iteration of the backward-Euler step."""
+        kf, kr, n_old, y, dt = _f64(kf), _f64(kr), _f64(n_old), _f64(y), _f64(dt)
+        ld = y.shape[1]
+        ncol = ld if ncol is None else ncol
+        s, keep = self._net(net)
+        delta, y_new = np.zeros_like(y), np.zeros_like(y)
+        rc = self.lib.orc_newton_step(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(kf), _ptr(kr), _ptr(n_old),
+                                      _ptr(dt), _ptr(y), _ptr(delta), _ptr(y_new))
+        if rc != 0:
+            raise ArithmeticError("oracle Newton step failed (%d: -2 = singular matrix)" % rc)
+        return delta, y_new

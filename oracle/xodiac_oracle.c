@@ -421,3 +421,104 @@ long orc_jac_pattern(const orc_network *net, long *row_ptr, int *col) {
   free(m);
   return k;
 }
+
+/* ---------------------------------------------------------------- f1: implicit (backward-Euler) Newton step
+ * The paper's continuity equation "is a stiff ordinary differential equation (ODE), implicit solvers
+ * are the most suitable choice ... the lower-order backward Euler method (Hu et al. 2012), the
+ * higher-order DLSODES solver".  One backward-Euler step of size dt from n_old solves
+ *     F(y) = y - n_old - dt f(y) = 0,        f = dn/dt of O5 (chemistry only; transport is off the path)
+ * and one Newton iteration from the iterate y is
+ *     (I - dt Jac(y)) delta = -F(y),          y_new = y + delta,      Jac of O6.
+ * The oracle is that definition written out for ONE column at a time: f from orc_source (rounded to
+ * double, as the library's xod_source returns it), Jac as the dense matrix of O6 in real_t, and the
+ * linear system solved by plain dense Gaussian elimination with partial pivoting in real_t.  No
+ * sparsity, no ordering, no reuse of factors.
+ * Pins (tests/test_oracle_newton.py): the closed form n0/(1 + dt k) of a first-order decay; a 2 x 2
+ * reversible pair solved by hand; numpy's solver on the exported system; a^T delta = -a^T (y - n_old)
+ * for every element; delta = 0 at the equilibrium fixed point; delta/dt -> f as dt -> 0; quadratic
+ * convergence of the iteration to F = 0. */
+
+/* A [ns][ns] row-major and b [ns] of column c:  A = I - dt Jac(y), b = -(y - n_old - dt f(y)) */
+static int newton_system_real(const orc_network *net, long ld, const double *kf, const double *kr,
+                              const double *n_old, const double *dt, const double *y, long c,
+                              real_t *A, real_t *b, real_t *scratch /* ns*ns */) {
+  long ns = net->n_species;
+  double *col = (double *)malloc(sizeof(double) * (size_t)(ns * 2 + 2 * net->n_reactions + 1));
+  if (!col) return -1;
+  double *yc = col, *fc = col + ns, *kfc = fc + ns, *krc = kfc + net->n_reactions;
+  for (long i = 0; i < ns; ++i) yc[i] = y[i * ld + c];
+  for (long r = 0; r < net->n_reactions; ++r) kfc[r] = kf[r * ld + c], krc[r] = kr[r * ld + c];
+  if (orc_source(net, 1, 1, kfc, krc, yc, fc, NULL, NULL) != 0) { free(col); return -1; }
+  jacobian_dense_real(net, 1, kfc, krc, yc, 0, A, scratch);
+  real_t h = (real_t)dt[c];
+  for (long i = 0; i < ns; ++i) {
+    for (long j = 0; j < ns; ++j) A[i * ns + j] = (i == j ? (real_t)1 : (real_t)0) - h * A[i * ns + j];
+    b[i] = -((real_t)yc[i] - (real_t)n_old[i * ld + c] - h * (real_t)fc[i]);
+  }
+  free(col);
+  return 0;
+}
+
+/* dense Gaussian elimination with partial pivoting; A is destroyed, x = A^-1 b.  Returns -1 if singular. */
+static int solve_dense_real(long n, real_t *A, real_t *b, real_t *x) {
+  for (long k = 0; k < n; ++k) {
+    long p = k;
+    for (long i = k + 1; i < n; ++i)
+      if (R_FABS(A[i * n + k]) > R_FABS(A[p * n + k])) p = i;
+    if (A[p * n + k] == 0) return -1;
+    if (p != k) {
+      for (long j = 0; j < n; ++j) { real_t t = A[k * n + j]; A[k * n + j] = A[p * n + j]; A[p * n + j] = t; }
+      real_t t = b[k]; b[k] = b[p]; b[p] = t;
+    }
+    for (long i = k + 1; i < n; ++i) {
+      real_t l = A[i * n + k] / A[k * n + k];
+      if (l == 0) continue;
+      for (long j = k + 1; j < n; ++j) A[i * n + j] -= l * A[k * n + j];
+      b[i] -= l * b[k];
+    }
+  }
+  for (long i = n - 1; i >= 0; --i) {
+    real_t s = b[i];
+    for (long j = i + 1; j < n; ++j) s -= A[i * n + j] * x[j];
+    x[i] = s / A[i * n + i];
+  }
+  return 0;
+}
+
+/* The system of column c, rounded to double (tests form residuals and call a library solver on it). */
+int orc_newton_system(const orc_network *net, long ld, const double *kf, const double *kr,
+                      const double *n_old, const double *dt, const double *y, long c, double *A_out,
+                      double *b_out) {
+  long ns = net->n_species;
+  real_t *A = (real_t *)malloc(sizeof(real_t) * (size_t)(2 * ns * ns + ns));
+  if (!A) return -1;
+  real_t *S = A + ns * ns, *b = S + ns * ns;
+  int rc = newton_system_real(net, ld, kf, kr, n_old, dt, y, c, A, b, S);
+  if (rc == 0) {
+    for (long e = 0; e < ns * ns; ++e) A_out[e] = (double)A[e];
+    for (long i = 0; i < ns; ++i) b_out[i] = (double)b[i];
+  }
+  free(A);
+  return rc;
+}
+
+/* delta, y_new: [n_species][ld]; either may be NULL.  Returns 0, -1 (memory) or -2 (singular matrix). */
+int orc_newton_step(const orc_network *net, long ncol, long ld, const double *kf, const double *kr,
+                    const double *n_old, const double *dt, const double *y, double *delta, double *y_new) {
+  long ns = net->n_species;
+  real_t *A = (real_t *)malloc(sizeof(real_t) * (size_t)(2 * ns * ns + 2 * ns));
+  if (!A) return -1;
+  real_t *S = A + ns * ns, *b = S + ns * ns, *x = b + ns;
+  int rc = 0;
+  for (long c = 0; c < ncol && rc == 0; ++c) {
+    rc = newton_system_real(net, ld, kf, kr, n_old, dt, y, c, A, b, S);
+    if (rc == 0 && solve_dense_real(ns, A, b, x) != 0) rc = -2;
+    if (rc != 0) break;
+    for (long i = 0; i < ns; ++i) {
+      if (delta) delta[i * ld + c] = (double)x[i];
+      if (y_new) y_new[i * ld + c] = (double)((real_t)y[i * ld + c] + x[i]);
+    }
+  }
+  free(A);
+  return rc;
+}
