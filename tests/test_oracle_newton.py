@@ -152,6 +152,8 @@ def test_solution_agrees_with_a_library_solver_on_the_same_system(oracle, networ
         x = np.linalg.solve(A, b)
         cond = np.linalg.cond(A)
         assert np.all(np.abs(x - delta[:, c]) <= 1e-15 * cond * np.abs(delta[:, c]).max() + 1e-300)
-        # residual evaluated in double: its own rounding is bounded by (ns + 2) eps (|A| |delta| + |b|)
+        # Gaussian elimination with partial pivoting is backward stable NORMWISE (densities span 40 decades, so
+        # a componentwise bound does not hold for the small rows); the residual is evaluated in double here
         r = A @ delta[:, c] - b
-        assert np.all(np.abs(r) <= (net.n_species + 2) * 2.3e-16 * (np.abs(A) @ np.abs(delta[:, c]) + np.abs(b)))
+        bound = np.abs(A).sum(axis=1).max() * np.abs(delta[:, c]).max() + np.abs(b).max()
+        assert np.abs(r).max() <= (net.n_species + 2) * 2.3e-16 * bound
