@@ -60,7 +60,10 @@ typedef enum {
  * non-falloff reactions with one / two-or-three listed reactants. */
 enum { XOD_UNI = 0, XOD_BI = 1, XOD_FALLOFF = 2, XOD_PHOTO = 3 };
 
-enum { XOD_FLAG_SKIP_BALANCE_CHECK = 1u };
+enum {
+  XOD_FLAG_SKIP_BALANCE_CHECK = 1u,
+  XOD_FLAG_BUILD_LU = 2u /* also build the symbolic LU of the Jacobian pattern (needed by xod_newton_step) */
+};
 
 typedef struct {
   int32_t n_species, n_elements, n_reactions;
@@ -145,7 +148,8 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
  * be NULL.  Synchronises on the last recorded event, then clears the record. */
 enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD_KERNEL_RATES_FROM_K = 3,
        XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
-       XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_JAC_TILED = 9, XOD_KERNEL_COUNT = 10 };
+       XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_JAC_TILED = 9, XOD_KERNEL_NEWTON_ASSEMBLE = 10,
+       XOD_KERNEL_LU_FACTOR = 11, XOD_KERNEL_LU_SOLVE = 12, XOD_KERNEL_COUNT = 13 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);
@@ -195,6 +199,33 @@ xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, co
  * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, ncol > 2097120), XOD_ERR_CUDA. */
 xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
                         const double *kr, const double *n, double *jac, void *stream);
+
+/* ---- f1: one Newton iteration of a backward-Euler step, batched over columns.
+ * "The discretized continuity equation is a stiff ordinary differential equation (ODE), implicit solvers are
+ * the most suitable choice ... the lower-order backward Euler method ... the higher-order DLSODES solver"
+ * (PAPER.md:85).  With f = dn/dt (Eq. 1 without transport) and Jac its Jacobian, a backward-Euler step of
+ * size dt from n_old solves F(y) = y - n_old - dt f(y) = 0; this call performs
+ *     (I - dt Jac(y)) delta = -F(y),     y <- y + delta
+ * for every column: f(y) by the kernels of xod_source, Jac(y) by those of xod_jacobian, then a sparse LU
+ * without pivoting in a fixed minimum-degree order (one symbolic factorisation per network, built at create
+ * with XOD_FLAG_BUILD_LU; the numeric factorisation runs with columns as lanes) and the two triangular
+ * solves.  Iterate the call until delta is small; with dt[c] = gamma it is also the Newton step of a BDF
+ * formula whose history terms the caller folds into n_old.
+ * kf, kr [n_reactions][ld] (xod_rate_coeffs; T, P are fixed during a step), n_old, y [n_species][ld], dt [ld]
+ * (per column, seconds), delta [n_species][ld] optional (NULL to skip): device memory owned by the caller; y is
+ * updated in place; workspace >= xod_newton_workspace_bytes(net, ncol) (columns are processed 2 048 at a time).
+ * A zero pivot gives IEEE inf/NaN in that column (no pivoting, no error).
+ * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, network created without XOD_FLAG_BUILD_LU or without the
+ * single-kernel tables), XOD_ERR_WORKSPACE, XOD_ERR_CUDA.
+ * xod_network_lu_info: info[5] = enabled, nonzeros of L + U (with fill), (row, pivot) pairs, multiply-add
+ * updates of one factorisation, longest row.  xod_network_lu_pattern: perm[p] = species eliminated p-th;
+ * row p of the filled pattern = permuted column indices, ascending (L part, diagonal, U part). */
+xod_status xod_network_lu_info(const xod_network *net, int64_t *info);
+xod_status xod_network_lu_pattern(const xod_network *net, int32_t *perm, int64_t *row_ptr, int32_t *col);
+size_t xod_newton_workspace_bytes(const xod_network *net, int64_t ncol);
+xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                           const double *n_old, const double *dt, double *y, double *delta, void *workspace,
+                           size_t workspace_bytes, void *stream);
 
 /* ---- end-to-end convenience: the fused call on HOST buffers (pinned for overlap; pageable works
  * but serialises).  Columns are processed in chunks of one round of tiles per SM through three

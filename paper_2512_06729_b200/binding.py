@@ -15,9 +15,9 @@ _lib = None
 
 XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
-XOD_FLAG_SKIP_BALANCE_CHECK = 1
+XOD_FLAG_SKIP_BALANCE_CHECK, XOD_FLAG_BUILD_LU = 1, 2
 XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL, XOD_TUNE_JAC_TILED = 0, 1, 2, 3, 4
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled"]
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -27,7 +27,8 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_rate_coeffs_workspace_bytes", "xod_rate_coeffs", "xod_source_workspace_bytes",
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
            "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params",
-           "xod_check_status", "xod_build_has_checks", "xod_network_jac_info"]
+           "xod_check_status", "xod_build_has_checks", "xod_network_jac_info", "xod_network_lu_info", "xod_network_lu_pattern",
+           "xod_newton_workspace_bytes", "xod_newton_step"]
 
 
 class XodError(RuntimeError):
@@ -55,7 +56,7 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         L.xod_last_error.restype = C.c_char_p
         for name in ("xod_rate_coeffs_workspace_bytes", "xod_source_workspace_bytes",
-                     "xod_source_fused_workspace_bytes"):
+                     "xod_source_fused_workspace_bytes", "xod_newton_workspace_bytes"):
             getattr(L, name).restype = C.c_size_t
             getattr(L, name).argtypes = [C.c_void_p, C.c_int64]
         L.xod_launch_count.restype = C.c_int64
@@ -161,6 +162,19 @@ class Network:
         keys = ("enabled", "chunk", "nchunk", "units", "acc_rows", "smem_bytes", "slots", "entries")
         return dict(zip(keys, [int(x) for x in v]))
 
+    def lu_info(self):
+        v = (C.c_int64 * 5)()
+        _check(lib().xod_network_lu_info(self._h, v))
+        return dict(zip(("enabled", "nnz_lu", "pairs", "updates", "max_row"), [int(x) for x in v]))
+
+    def lu_pattern(self):
+        info = self.lu_info()
+        perm = np.zeros(self.n_species, dtype=np.int32)
+        rp = np.zeros(self.n_species + 1, dtype=np.int64)
+        col = np.zeros(info["nnz_lu"], dtype=np.int32)
+        _check(lib().xod_network_lu_pattern(self._h, _hp(perm), _hp(rp), _hp(col)))
+        return perm, rp, col
+
     def fused_params(self, interval):
         """(user_rxn [npad], kind [npad], coef [npad][16], breakpoints) of one thermo interval."""
         info = self.fused_info()
@@ -224,6 +238,15 @@ class Network:
     def jacobian(self, ncol, ld, kf, kr, n, jac, stream=None):
         _check(lib().xod_jacobian(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(kf), _dp(kr), _dp(n),
                                   _dp(jac), _stream(stream)))
+
+    # ---- f1: one Newton iteration of a backward-Euler step (y updated in place)
+    def newton_workspace_bytes(self, ncol):
+        return lib().xod_newton_workspace_bytes(self._h, ncol)
+
+    def newton_step(self, ncol, ld, kf, kr, n_old, dt, y, delta=None, workspace=None, stream=None):
+        _check(lib().xod_newton_step(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(kf), _dp(kr), _dp(n_old), _dp(dt),
+                                     _dp(y), _dp(delta), _dp(workspace),
+                                     C.c_size_t(0 if workspace is None else workspace.numel() * 8), _stream(stream)))
 
     # ---- end to end on HOST buffers (numpy arrays or pinned torch CPU tensors)
     def source_fused_host(self, ncol, ld, T, P, J, n, dndt):

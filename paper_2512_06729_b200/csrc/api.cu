@@ -9,6 +9,7 @@
 
 #include "fused.cuh"
 #include "jac_tiled.cuh"
+#include "newton.cuh"
 #include "rates2.cuh"
 #include "kernels.cuh"
 
@@ -184,6 +185,13 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (net->h.jt.enabled && jac_tiled_smem_bytes(net->h.ns, net->h.jt.acc_rows, chunk, net->h.jt.meta_cap) <= kFusedSmemMax) break;
       net->h.jt.enabled = false;
     }
+    if (desc->flags & XOD_FLAG_BUILD_LU) {
+      pack_lu(net->h);
+      if (!net->h.lu.enabled) {
+        delete net;
+        return fail(XOD_ERR_INVALID_ARG, "XOD_FLAG_BUILD_LU: the LU tables do not fit (too many species or too much fill)");
+      }
+    }
   } catch (const std::bad_alloc &) {
     delete net;
     return fail(XOD_ERR_ALLOC, "out of host memory while packing");
@@ -254,6 +262,23 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (st == XOD_OK) {
         cudaError_t ce = cudaFuncSetAttribute(k_jac_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
         if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_jac_tiled)");
+      }
+    }
+    if (h.lu.enabled) {
+      LuHost &u = h.lu;
+      LuDev &ud = net->ld;
+      ud.enabled = 1, ud.n = u.n, ud.max_row = u.max_row, ud.nnz = u.nnz;
+      if (st == XOD_OK) st = upload(net, u.perm, &ud.perm);
+      if (st == XOD_OK) st = upload(net, u.diag, &ud.diag);
+      if (st == XOD_OK) st = upload(net, u.src, &ud.src);
+      if (st == XOD_OK) st = upload(net, u.col, &ud.col);
+      if (st == XOD_OK) st = upload(net, u.row_ptr, &ud.row_ptr);
+      if (st == XOD_OK) st = upload(net, u.rows, &ud.rows);
+      if (st == XOD_OK) st = upload(net, u.pairs, &ud.pairs);
+      if (st == XOD_OK) st = upload(net, u.tgt, &ud.tgt);
+      if (st == XOD_OK) {
+        cudaError_t ce = cudaFuncSetAttribute(k_lu_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
+        if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_lu_factor)");
       }
     }
 #undef UP
@@ -487,17 +512,18 @@ size_t fused_partial_bytes(const xod_network *net, int64_t ncol) {
 // T, P, J given: xod_source_fused (coefficients evaluated in the kernel); kf, kr given: xod_source
 xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T, const double *P,
                         const double *J, const double *kf, const double *kr, const double *n, double *dndt,
-                        void *workspace, cudaStream_t s) {
+                        void *workspace, cudaStream_t s, int64_t ldo = 0 /* pitch of dndt; 0: ld */) {
+  if (ldo == 0) ldo = ld;
   const HostTables &h = net->h;
   auto off = [](const double *p, int64_t c) { return p ? p + c : p; };
   if (const int64_t c_full = fused_full_round_cols(net, ncol)) {  // columns are independent: two sub-ranges
-    xod_status st = launch_fused(net, c_full, ld, T, P, J, kf, kr, n, dndt, workspace, s);
+    xod_status st = launch_fused(net, c_full, ld, T, P, J, kf, kr, n, dndt, workspace, s, ldo);
     if (st != XOD_OK) return st;
     return launch_fused(net, ncol - c_full, ld, off(T, c_full), off(P, c_full), off(J, c_full), off(kf, c_full),
-                        off(kr, c_full), n + c_full, dndt + c_full, workspace, s);
+                        off(kr, c_full), n + c_full, dndt + c_full, workspace, s, ldo);
   }
   FusedArgs a{};
-  a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.J = J, a.n = n, a.kf = kf, a.kr = kr;
+  a.ncol = ncol, a.ld = ld, a.ldo = ldo, a.T = T, a.P = P, a.J = J, a.n = n, a.kf = kf, a.kr = kr;
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
   a.nsplit = fused_split(net, ncol);
   a.log2_kb = kLog2Kb;
@@ -519,9 +545,35 @@ xod_status launch_fused(const xod_network *net, int64_t ncol, int64_t ld, const 
   if (a.nsplit > 1) {
     dim3 g((unsigned)((ncol + 127) / 128), (unsigned)h.ns);
     Timed tm(net, KID_FUSED_COMBINE, s);
-    k_fused_combine<<<g, 128, 0, s>>>(h.ns, ncol, ld, a.ldp, a.nsplit, part, dndt);
+    k_fused_combine<<<g, 128, 0, s>>>(h.ns, ncol, ldo, a.ldp, a.nsplit, part, dndt);
   }
   XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+// k_jac_tiled: whole rounds of column tiles on every SM run unsplit; the last partial round (or a batch with
+// fewer tiles than SMs) has each tile's units split over the otherwise idle SMs (units are independent)
+xod_status launch_jac_tiled(const xod_network *net, int64_t ncol, int64_t ld, int64_t ldo, const double *kf,
+                            const double *kr, const double *n, double *jac, cudaStream_t s) {
+  const size_t smem = jac_tiled_smem_bytes(net->h.ns, net->h.jt.acc_rows, net->h.jt.chunk, net->h.jt.meta_cap);
+  const int64_t ntiles = (ncol + kFW - 1) / kFW, sm = net->sm_count;
+  const int64_t full = net->force_split > 0 ? 0 : ntiles / sm * sm;
+  for (int part = 0; part < 2; ++part) {
+    const int64_t t0 = part == 0 ? 0 : full, t1 = part == 0 ? full : ntiles;
+    if (t1 <= t0) continue;
+    JacArgs a{};
+    const int64_t c0 = t0 * kFW;
+    a.ncol = std::min<int64_t>(ncol, t1 * kFW) - c0, a.ld = ld, a.ldo = ldo;
+    a.kf = kf + c0, a.kr = kr + c0, a.n = n + c0, a.jac = jac + c0;
+    a.ntiles = (int32_t)(t1 - t0);
+    const int64_t split = part == 0 ? 1 : (net->force_split > 0 ? net->force_split : sm / (t1 - t0));
+    a.nsplit = (int32_t)std::max<int64_t>(1, std::min<int64_t>(split, net->h.jt.n_units));
+    a.nr = net->h.nr, a.nnz = net->d.nnz_jac;
+    const unsigned grid = (unsigned)std::min<int64_t>((int64_t)a.ntiles * a.nsplit, sm);
+    Timed tm(net, KID_JAC_TILED, s);
+    k_jac_tiled<<<grid, kFWarps * 32, smem, s>>>(net->jd, net->h.ns, a);
+    XOD_CUDA(cudaGetLastError());
+  }
   return XOD_OK;
 }
 
@@ -662,30 +714,7 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
   if (!n || !jac) return fail(XOD_ERR_INVALID_ARG, "n or jac is NULL");
   if (net->h.nr > 0 && (!kf || !kr)) return fail(XOD_ERR_INVALID_ARG, "kf or kr is NULL");
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if (net->jd.enabled && net->use_jac_tiled && net->h.nr > 0) {
-    // whole rounds of column tiles on every SM run unsplit; the last partial round (or a batch with fewer
-    // tiles than SMs) has each tile's units split over the otherwise idle SMs (units are independent)
-    const size_t smem = jac_tiled_smem_bytes(net->h.ns, net->h.jt.acc_rows, net->h.jt.chunk, net->h.jt.meta_cap);
-    const int64_t ntiles = (ncol + kFW - 1) / kFW, sm = net->sm_count;
-    const int64_t full = net->force_split > 0 ? 0 : ntiles / sm * sm;
-    for (int part = 0; part < 2; ++part) {
-      const int64_t t0 = part == 0 ? 0 : full, t1 = part == 0 ? full : ntiles;
-      if (t1 <= t0) continue;
-      JacArgs a{};
-      const int64_t c0 = t0 * kFW;
-      a.ncol = std::min<int64_t>(ncol, t1 * kFW) - c0, a.ld = ld;
-      a.kf = kf + c0, a.kr = kr + c0, a.n = n + c0, a.jac = jac + c0;
-      a.ntiles = (int32_t)(t1 - t0);
-      int64_t split = part == 0 ? 1 : (net->force_split > 0 ? net->force_split : sm / (t1 - t0));
-      a.nsplit = (int32_t)std::max<int64_t>(1, std::min<int64_t>(split, net->h.jt.n_units));
-      a.nr = net->h.nr, a.nnz = net->d.nnz_jac;
-      const unsigned grid = (unsigned)std::min<int64_t>((int64_t)a.ntiles * a.nsplit, sm);
-      Timed tm(net, KID_JAC_TILED, s);
-      k_jac_tiled<<<grid, kFWarps * 32, smem, s>>>(net->jd, net->h.ns, a);
-      XOD_CUDA(cudaGetLastError());
-    }
-    return XOD_OK;
-  }
+  if (net->jd.enabled && net->use_jac_tiled && net->h.nr > 0) return launch_jac_tiled(net, ncol, ld, ld, kf, kr, n, jac, s);
   const int64_t ncg = (ncol + 31) / 32;
   if (ncg > 65535) return fail(XOD_ERR_INVALID_ARG, "ncol too large for one xod_jacobian call (max 2097120)");
   const int64_t want = (net->d.nnz_jac + 7) / 8;
@@ -768,6 +797,91 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
   }
 #undef XOD_CUDA_DRAIN
   for (int i = 0; i < kHostSlots; ++i) XOD_CUDA(cudaStreamSynchronize(static_cast<cudaStream_t>(net->host_streams[i])));
+  return XOD_OK;
+}
+
+// ---------------------------------------------------------------------------- f1: implicit step
+
+xod_status xod_network_lu_info(const xod_network *net, int64_t *info) {
+  if (!net || !info) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
+  const LuHost &u = net->h.lu;
+  info[0] = u.enabled, info[1] = u.nnz, info[2] = (int64_t)u.pairs.size(), info[3] = u.n_updates, info[4] = u.max_row;
+  return XOD_OK;
+}
+
+xod_status xod_network_lu_pattern(const xod_network *net, int32_t *perm, int64_t *row_ptr, int32_t *col) {
+  if (!net) return fail(XOD_ERR_INVALID_ARG, "net is NULL");
+  const LuHost &u = net->h.lu;
+  if (!u.enabled) return fail(XOD_ERR_INVALID_ARG, "the network was created without XOD_FLAG_BUILD_LU");
+  if (perm) std::memcpy(perm, u.perm.data(), u.perm.size() * sizeof(int32_t));
+  if (row_ptr) std::memcpy(row_ptr, u.row_ptr.data(), u.row_ptr.size() * sizeof(int64_t));
+  if (col) std::memcpy(col, u.col.data(), u.col.size() * sizeof(int32_t));
+  return XOD_OK;
+}
+
+}  // extern "C"
+
+namespace {
+constexpr int64_t kNewtonChunk = 2048;   // columns per pass of the implicit step (bounds the workspace)
+int64_t newton_chunk(int64_t ncol) { return std::min<int64_t>(round_up(std::max<int64_t>(ncol, 1), 32), kNewtonChunk); }
+}  // namespace
+
+extern "C" {
+
+size_t xod_newton_workspace_bytes(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0 || !net->h.lu.enabled) return 0;
+  const int64_t cw = newton_chunk(ncol);
+  const size_t rows = (size_t)2 * net->h.ns + (size_t)net->h.jac_col.size() + (size_t)net->h.lu.nnz;
+  return rows * (size_t)cw * sizeof(double) + fused_partial_bytes(net, cw) + 1024;
+}
+
+xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                           const double *n_old, const double *dt, double *y, double *delta, void *workspace,
+                           size_t workspace_bytes, void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (!net->h.lu.enabled) return fail(XOD_ERR_INVALID_ARG, "the network was created without XOD_FLAG_BUILD_LU");
+  if (!net->fd.enabled || !net->jd.enabled || net->h.nr == 0)
+    return fail(XOD_ERR_INVALID_ARG, "the implicit step needs the single-kernel source and Jacobian tables (see xod_network_fused_info, xod_network_jac_info)");
+  if (ncol == 0) return XOD_OK;
+  if (!kf || !kr || !n_old || !dt || !y) return fail(XOD_ERR_INVALID_ARG, "kf, kr, n_old, dt or y is NULL");
+  if (!workspace || workspace_bytes < xod_newton_workspace_bytes(net, ncol))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_newton_workspace_bytes");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int64_t cw = newton_chunk(ncol);
+  const size_t ns = net->h.ns, nnzj = net->h.jac_col.size(), nnzl = (size_t)net->h.lu.nnz;
+  double *f = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
+  double *rhs = f + ns * cw, *jac = rhs + ns * cw, *lu = jac + nnzj * cw;
+  void *src_ws = lu + nnzl * cw;
+  const size_t smem = (size_t)net->h.lu.max_row * 32 * sizeof(double);
+  if (smem > kFusedSmemMax) return fail(XOD_ERR_INVALID_ARG, "a row of the LU pattern does not fit shared memory");
+  for (int64_t c0 = 0; c0 < ncol; c0 += cw) {
+    const int64_t w = std::min(cw, ncol - c0);
+    // f(y) and Jac(y) of this chunk into the workspace (pitch cw), by the kernels of xod_source / xod_jacobian
+    if ((st = launch_fused(net, w, ld, nullptr, nullptr, nullptr, kf + c0, kr + c0, y + c0, f, src_ws, s, cw)) != XOD_OK) return st;
+    if ((st = launch_jac_tiled(net, w, ld, cw, kf + c0, kr + c0, y + c0, jac, s)) != XOD_OK) return st;
+    NewtonArgs a{};
+    a.ncol = w, a.ld = ld, a.ldw = cw;
+    a.n_old = n_old + c0, a.dt = dt + c0, a.f = f, a.jac = jac, a.y = y + c0, a.delta = delta ? delta + c0 : nullptr;
+    a.lu = lu, a.rhs = rhs, a.nnz_jac = (int64_t)nnzj;
+    {
+      const int64_t gx = (w + 127) / 128;
+      dim3 grid((unsigned)gx, (unsigned)std::max<int64_t>(1, std::min<int64_t>(net->h.lu.nnz, (int64_t)net->sm_count * 16 / gx)));
+      Timed tm(net, KID_NEWTON_ASSEMBLE, s);
+      k_newton_assemble<<<grid, 128, 0, s>>>(net->ld, a);
+      XOD_CUDA(cudaGetLastError());
+    }
+    {
+      Timed tm(net, KID_LU_FACTOR, s);
+      k_lu_factor<<<(unsigned)((w + 31) / 32), 32 * kLuWarps, smem, s>>>(net->ld, lu, cw, w);
+      XOD_CUDA(cudaGetLastError());
+    }
+    {
+      Timed tm(net, KID_LU_SOLVE, s);
+      k_lu_solve<<<(unsigned)((w + 127) / 128), 128, 0, s>>>(net->ld, a);
+      XOD_CUDA(cudaGetLastError());
+    }
+  }
   return XOD_OK;
 }
 

@@ -33,7 +33,8 @@
 namespace xod {
 
 struct FusedArgs {
-  int64_t ncol, ld;           // caller's columns and row pitch
+  int64_t ncol, ld;           // caller's columns and the row pitch of the inputs
+  int64_t ldo;                // row pitch of dndt (= ld in the public calls; the implicit step writes into its workspace)
   const double *T, *P, *J, *n;
   const double *kf, *kr;      // FROMK only: stored coefficients [n_reactions][ld]
   double *out;                // nsplit == 1: dndt [ns][ld]; else partial sums [nsplit][ns][ldp]
@@ -218,7 +219,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       const int c = tid & (kFW - 1);
       if (col0 + c < a.ncol) {
         double *o = a.nsplit == 1 ? a.out + col0 + c : a.out + (size_t)split * ns * a.ldp + col0 + c;
-        const int64_t pitch = a.nsplit == 1 ? a.ld : a.ldp;
+        const int64_t pitch = a.nsplit == 1 ? a.ldo : a.ldp;
         for (int i = tid >> 4; i < ns; i += (kFWarps * 32) >> 4) o[(size_t)i * pitch] = acc_s[i * kFW + c];
       }
     }

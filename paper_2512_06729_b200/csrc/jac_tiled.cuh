@@ -27,8 +27,9 @@ namespace xod {
 
 struct JacArgs {
   int64_t ncol, ld;
+  int64_t ldo;                 // row pitch of jac (= ld in the public call)
   const double *kf, *kr, *n;   // [n_reactions][ld] x 2 (USER order), [ns][ld]
-  double *jac;                 // [nnz_jac][ld]
+  double *jac;                 // [nnz_jac][ldo]
   int32_t ntiles, nsplit;      // column tiles; CTAs a tile's chunks are split over (at unit boundaries)
   int32_t nr;                  // rows of kf / kr
   int64_t nnz;                 // rows of jac
@@ -104,7 +105,7 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_jac_tiled(JacTiledDev f, in
           double sum = r[0];
           r[0] = 0.0;
           for (int x = 1; x < e.z; ++x) sum += r[x * kFW], r[x * kFW] = 0.0;
-          if (valid) a.jac[(size_t)XOD_IDX((int64_t)e.x, a.nnz) * a.ld + col0 + c] = sum;
+          if (valid) a.jac[(size_t)XOD_IDX((int64_t)e.x, a.nnz) * a.ldo + col0 + c] = sum;
         }
         // no barrier needed here: the next chunk's phase B touches these rows only after its own barrier
       }

@@ -1,0 +1,139 @@
+// pack_lu.cpp -- symbolic factorisation for the batched implicit step.
+//
+// The chemistry is a stiff ODE integrated implicitly; each Newton iteration of a
+// backward-Euler / BDF step solves (I - gamma Jac) delta = -F with the SAME sparsity for every
+// column, so the elimination order, the filled pattern and the whole update schedule are built once
+// here, on the host, and shared by all columns (the kernels of newton.cuh only stream values).
+//   * order: greedy minimum degree on the symmetric pattern of xod_network_jac_pattern (ties -> the
+//     lowest species index), which keeps hub species (H, H2, OH-like) for last;
+//   * pattern: the elimination graph with fill; row p = L part | diagonal | U part in permuted indices;
+//   * schedule (row-by-row "up-looking" LU without pivoting, as DLSODES' sparse solver does): for row i
+//     and every k in L(i) ascending,  l = a_ik / a_kk;  a_ij -= l a_kj for j in U(k);  the slots of
+//     those j inside row i are precomputed (tgt).
+#include <algorithm>
+#include <cstring>
+
+#include "xod_internal.h"
+
+namespace xod {
+
+void pack_lu(HostTables &h) {
+  LuHost &u = h.lu;
+  u = LuHost();
+  const int n = h.ns;
+  if (n <= 0 || n >= 0xffff) return;
+  // adjacency as a dense bit matrix (n <= 65534: at most 512 MB, the configs need 44 KB)
+  const size_t W = ((size_t)n + 63) / 64;
+  if ((double)W * n * 8 > 1.0e9) return;
+  std::vector<uint64_t> adj(W * n, 0);
+  auto set = [&](int a, int b) { adj[(size_t)a * W + (b >> 6)] |= 1ull << (b & 63); };
+  auto get = [&](int a, int b) { return (adj[(size_t)a * W + (b >> 6)] >> (b & 63)) & 1ull; };
+  auto clr = [&](int a, int b) { adj[(size_t)a * W + (b >> 6)] &= ~(1ull << (b & 63)); };
+  for (int i = 0; i < n; ++i)
+    for (int64_t e = h.jac_ptr[i]; e < h.jac_ptr[i + 1]; ++e) {
+      const int j = h.jac_col[e];
+      if (j != i) set(i, j), set(j, i);
+    }
+  std::vector<int> deg(n);
+  for (int i = 0; i < n; ++i) {
+    int d = 0;
+    for (size_t w = 0; w < W; ++w) d += __builtin_popcountll(adj[(size_t)i * W + w]);
+    deg[i] = d;
+  }
+  std::vector<char> alive(n, 1);
+  u.perm.resize(n), u.pos_of.resize(n);
+  std::vector<std::vector<int>> urow(n);  // U(p) as species indices, filled at elimination time
+  for (int p = 0; p < n; ++p) {
+    int best = -1;
+    for (int i = 0; i < n; ++i)
+      if (alive[i] && (best < 0 || deg[i] < deg[best])) best = i;
+    u.perm[p] = best, u.pos_of[best] = p;
+    alive[best] = 0;
+    std::vector<int> &nb = urow[p];
+    for (size_t w = 0; w < W; ++w) {
+      uint64_t bits = adj[(size_t)best * W + w];
+      while (bits) {
+        const int b = __builtin_ctzll(bits);
+        bits &= bits - 1;
+        nb.push_back((int)(w * 64 + b));
+      }
+    }
+    for (int a : nb) clr(a, best), --deg[a];
+    for (size_t x = 0; x < nb.size(); ++x)
+      for (size_t y = x + 1; y < nb.size(); ++y)
+        if (!get(nb[x], nb[y])) set(nb[x], nb[y]), set(nb[y], nb[x]), ++deg[nb[x]], ++deg[nb[y]];
+  }
+  // rows in permuted indices: U(p) from the elimination, L(p) = {q < p : p in U(q)} by symmetry
+  std::vector<std::vector<int>> U(n), L(n);
+  for (int p = 0; p < n; ++p) {
+    for (int s : urow[p]) U[p].push_back(u.pos_of[s]);
+    std::sort(U[p].begin(), U[p].end());
+    for (int q : U[p]) L[q].push_back(p);   // p ascending, so every L row comes out sorted
+  }
+  u.n = n;
+  u.row_ptr.assign(n + 1, 0);
+  u.diag.resize(n);
+  for (int p = 0; p < n; ++p) {
+    u.diag[p] = (int32_t)(u.row_ptr[p] + (int64_t)L[p].size());
+    u.row_ptr[p + 1] = u.row_ptr[p] + (int64_t)L[p].size() + 1 + (int64_t)U[p].size();
+    u.max_row = std::max<int32_t>(u.max_row, (int32_t)(u.row_ptr[p + 1] - u.row_ptr[p]));
+  }
+  u.nnz = u.row_ptr[n];
+  if (u.nnz >= 0x7fffffff || u.max_row > 0xffff) {
+    u = LuHost();
+    return;
+  }
+  u.col.resize(u.nnz), u.src.assign(u.nnz, -1);
+  for (int p = 0; p < n; ++p) {
+    int64_t x = u.row_ptr[p];
+    for (int q : L[p]) u.col[x++] = q;
+    u.col[x++] = p;
+    for (int q : U[p]) u.col[x++] = q;
+  }
+  // where the Jacobian entries land (the rest is fill)
+  {
+    std::vector<int32_t> slot(n, -1);   // permuted column -> storage position, for the current row
+    for (int p = 0; p < n; ++p) {
+      for (int64_t x = u.row_ptr[p]; x < u.row_ptr[p + 1]; ++x) slot[u.col[x]] = (int32_t)x;
+      const int i = u.perm[p];
+      for (int64_t e = h.jac_ptr[i]; e < h.jac_ptr[i + 1]; ++e)   // bit 30 marks the diagonal (the "I" of I - gamma Jac)
+        u.src[slot[u.pos_of[h.jac_col[e]]]] = (int32_t)e | (h.jac_col[e] == i ? kLuDiagBit : 0);
+      for (int64_t x = u.row_ptr[p]; x < u.row_ptr[p + 1]; ++x) slot[u.col[x]] = -1;
+    }
+  }
+  // update schedule
+  u.rows.resize(n);
+  {
+    std::vector<int32_t> slot(n, -1);   // permuted column -> slot inside row i
+    for (int i = 0; i < n; ++i) {
+      const int64_t b = u.row_ptr[i], len = u.row_ptr[i + 1] - b;
+      for (int64_t x = 0; x < len; ++x) slot[u.col[b + x]] = (int32_t)x;
+      LuRow r;
+      r.begin = (int32_t)b, r.len = (int32_t)len, r.pair_begin = (int32_t)u.pairs.size();
+      for (size_t a = 0; a < L[i].size(); ++a) {
+        const int k = L[i][a];
+        LuPair pr;
+        pr.t_k = (int32_t)a, pr.diag_k = u.diag[k], pr.cnt = (int32_t)U[k].size(), pr.tgt_off = (int32_t)u.tgt.size();
+        if (u.tgt.size() + U[k].size() >= 0x7fffffffu) {
+          u = LuHost();
+          return;
+        }
+        for (int j : U[k]) {
+          if (slot[j] < 0) {   // cannot happen: (i, j) is in the filled pattern whenever k is in L(i) and j in U(k)
+            u = LuHost();
+            return;
+          }
+          u.tgt.push_back((uint16_t)slot[j]);
+        }
+        u.n_updates += pr.cnt;
+        u.pairs.push_back(pr);
+      }
+      r.pair_end = (int32_t)u.pairs.size();
+      u.rows[i] = r;
+      for (int64_t x = 0; x < len; ++x) slot[u.col[b + x]] = -1;
+    }
+  }
+  u.enabled = true;
+}
+
+}  // namespace xod

@@ -137,6 +137,35 @@ struct JacTiledDev {
   const int4 *meta, *slots, *chunk_info, *flush;
 };
 
+// ---- tables of the batched implicit step (f1: xod_newton_step; pack_lu.cpp, newton.cuh) ---------
+// Symbolic LU of the Jacobian pattern (symmetric, with diagonal) in a minimum-degree elimination order,
+// shared by all columns; values live in a [nnz_lu][cols] array, rows in elimination order, each row
+// stored as  L part (ascending) | diagonal | U part (ascending).
+constexpr int32_t kLuDiagBit = 1 << 30;   // in LuHost::src: the position is a diagonal
+constexpr int kLuWarps = 16;              // warps of a k_lu_factor CTA (32 columns x kLuWarps slices of the update loop)
+struct LuRow { int32_t begin, len, pair_begin, pair_end; };           // storage range of the row, its (i, k) pairs
+struct LuPair { int32_t t_k, diag_k, cnt, tgt_off; };                 // slot of a_ik in row i; diagonal of row k; |U(k)|; targets
+struct LuHost {
+  bool enabled = false;
+  int32_t n = 0, max_row = 0;
+  int64_t nnz = 0, n_updates = 0;
+  std::vector<int32_t> perm, pos_of;        // perm[p] = species eliminated p-th; pos_of[species] = p
+  std::vector<int64_t> row_ptr;             // [n + 1]
+  std::vector<int32_t> col, diag, src;      // [nnz] permuted column; [n] position of the diagonal; [nnz] Jacobian entry or -1 (fill)
+  std::vector<LuRow> rows;                  // [n]
+  std::vector<LuPair> pairs;                // sum_i |L(i)|, row by row, ascending k
+  std::vector<uint16_t> tgt;                // for pair (i, k): slot in row i of every column of U(k)
+};
+struct LuDev {
+  int32_t enabled, n, max_row;
+  int64_t nnz;
+  const int32_t *perm, *diag, *src, *col;
+  const int64_t *row_ptr;
+  const LuRow *rows;
+  const LuPair *pairs;
+  const uint16_t *tgt;
+};
+
 struct HostTables {
   int32_t ns = 0, ne = 0, nr = 0, n_photo = 0;
   int32_t uni_begin = 0, bi_begin = 0, fo_begin = 0, ph_begin = 0;
@@ -157,6 +186,7 @@ struct HostTables {
   std::vector<JacTerm> jac_terms;
   FusedHost f;
   JacTiledHost jt;
+  LuHost lu;
 };
 
 // one row task of a chunk schedule: an accumulator row and its entries (q row | nu bits)
@@ -175,6 +205,8 @@ size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap);
 // pack_jac.cpp: tables of the tiled Jacobian kernel for a given chunk size and accumulator-row budget
 void pack_jac_tiled(HostTables &h, int chunk, int acc_budget);
 bool check_jac_tiled(const HostTables &h, std::string &err);
+// pack_lu.cpp: minimum-degree ordering, filled pattern and update schedule of the implicit step
+void pack_lu(HostTables &h);
 size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 
 }  // namespace xod
@@ -182,7 +214,7 @@ size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused
@@ -198,6 +230,7 @@ struct xod_network {
   xod::DevTables d{};
   xod::FusedDev fd{};
   xod::JacTiledDev jd{};
+  xod::LuDev ld{};
   int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
   int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
   int64_t use_jac_tiled = 1;  // XOD_TUNE_JAC_TILED: 0 = the one-warp-per-entry gather kernel

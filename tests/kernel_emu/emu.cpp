@@ -18,6 +18,7 @@ void emu_syncthreads() { g_barrier->arrive_and_wait(); }
 #include "../../paper_2512_06729_b200/csrc/fused.cuh"
 #include "../../paper_2512_06729_b200/csrc/rates2.cuh"
 #include "../../paper_2512_06729_b200/csrc/jac_tiled.cuh"
+#include "../../paper_2512_06729_b200/csrc/newton.cuh"
 #include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
@@ -99,6 +100,7 @@ int emu_source_fused(const xod_network_desc *d, int64_t ncol, int64_t ld, const 
   a.nsplit = std::max(1, std::min(nsplit, (int)fd.nchunk));
   a.log2_kb = kLog2Kb;
   a.ldp = (ncol + 31) / 32 * 32;
+  a.ldo = ld;
   a.nr = h.nr, a.n_photo = h.n_photo;
   std::vector<double> part((size_t)a.nsplit * h.ns * a.ldp);
   a.out = a.nsplit == 1 ? dndt : part.data();
@@ -186,12 +188,69 @@ int emu_jacobian_tiled(const xod_network_desc *desc, int64_t ncol, int64_t ld, c
   jd.chunk_info = reinterpret_cast<const int4 *>(t.chunk_info.data());
   jd.flush = reinterpret_cast<const int4 *>(t.flush.data());
   JacArgs a{};
-  a.ncol = ncol, a.ld = ld, a.kf = kf, a.kr = kr, a.n = n, a.jac = jac;
+  a.ncol = ncol, a.ld = ld, a.ldo = ld, a.kf = kf, a.kr = kr, a.n = n, a.jac = jac;
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
   a.nsplit = std::max(1, std::min(nsplit, (int)t.n_units));
   a.nr = h.nr, a.nnz = (int64_t)h.jac_col.size();
   const int ns = h.ns;
   run_grid((unsigned)grid, 1, kFWarps * 32, true, [&] { k_jac_tiled(jd, ns, a); });
+  return 0;
+}
+
+// f1: one Newton iteration of the backward-Euler step, composed as xod_newton_step composes it: k_fused<true>
+// (f), k_jac_tiled (Jac), k_newton_assemble, k_lu_factor, k_lu_solve; workspace pitch ldw != ld on purpose
+int emu_newton_step(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                    const double *n_old, const double *dt, double *y, double *delta) {
+  HostTables h;
+  FusedDev fd;
+  std::string err;
+  if (!pack(desc, h, fd) || ncol <= 0) return 1;
+  for (int chunk : {4 * kFPass, 3 * kFPass, 2 * kFPass, kFPass}) {
+    const int64_t fixed = ((int64_t)(h.ns + 1) + 2 * (chunk + 1)) * kFW * 8 + 2 * 12 * 1024;
+    const int64_t budget = ((int64_t)kSmemMax - fixed) / (kFW * 8);
+    if (budget < 1) continue;
+    pack_jac_tiled(h, chunk, (int)std::min<int64_t>(budget, 0xfff0));
+    if (h.jt.enabled && jac_tiled_smem_bytes(h.ns, h.jt.acc_rows, chunk, h.jt.meta_cap) <= kSmemMax) break;
+    h.jt.enabled = false;
+  }
+  pack_lu(h);
+  if (!h.jt.enabled || !h.lu.enabled || (size_t)h.lu.max_row * 32 * 8 > kSmemMax) return 2;
+  const int ns = h.ns;
+  const int64_t ldw = (ncol + 31) / 32 * 32 + 32, nnzj = (int64_t)h.jac_col.size();
+  std::vector<double> f((size_t)ns * ldw, NAN), rhs((size_t)ns * ldw, NAN), jac((size_t)nnzj * ldw, NAN), lu((size_t)h.lu.nnz * ldw, NAN);
+  {  // f(y)
+    FusedArgs a{};
+    a.ncol = ncol, a.ld = ld, a.ldo = ldw, a.n = y, a.kf = kf, a.kr = kr;
+    a.ntiles = (int32_t)((ncol + kFW - 1) / kFW), a.nsplit = 1, a.log2_kb = kLog2Kb, a.ldp = ldw;
+    a.nr = h.nr, a.n_photo = h.n_photo, a.out = f.data();
+    run_grid(2, 1, kFWarps * 32, true, [&] { k_fused<true>(fd, ns, a); });
+  }
+  {  // Jac(y)
+    const JacTiledHost &t = h.jt;
+    JacTiledDev jd{};
+    jd.enabled = 1, jd.chunk = t.chunk, jd.nchunk = t.nchunk, jd.acc_rows = t.acc_rows, jd.meta_cap = t.meta_cap;
+    jd.n_flush = (int32_t)(t.flush.size() / 4);
+    jd.meta_ptr = t.meta_ptr.data();
+    jd.meta = reinterpret_cast<const int4 *>(t.meta.data());
+    jd.slots = reinterpret_cast<const int4 *>(t.slots.data());
+    jd.chunk_info = reinterpret_cast<const int4 *>(t.chunk_info.data());
+    jd.flush = reinterpret_cast<const int4 *>(t.flush.data());
+    JacArgs a{};
+    a.ncol = ncol, a.ld = ld, a.ldo = ldw, a.kf = kf, a.kr = kr, a.n = y, a.jac = jac.data();
+    a.ntiles = (int32_t)((ncol + kFW - 1) / kFW), a.nsplit = 1, a.nr = h.nr, a.nnz = nnzj;
+    run_grid(2, 1, kFWarps * 32, true, [&] { k_jac_tiled(jd, ns, a); });
+  }
+  const LuHost &u = h.lu;
+  LuDev ud{};
+  ud.enabled = 1, ud.n = u.n, ud.max_row = u.max_row, ud.nnz = u.nnz;
+  ud.perm = u.perm.data(), ud.diag = u.diag.data(), ud.src = u.src.data(), ud.col = u.col.data();
+  ud.row_ptr = u.row_ptr.data(), ud.rows = u.rows.data(), ud.pairs = u.pairs.data(), ud.tgt = u.tgt.data();
+  NewtonArgs a{};
+  a.ncol = ncol, a.ld = ld, a.ldw = ldw, a.n_old = n_old, a.dt = dt, a.f = f.data(), a.jac = jac.data();
+  a.y = y, a.delta = delta, a.lu = lu.data(), a.rhs = rhs.data(), a.nnz_jac = nnzj;
+  run_grid((unsigned)((ncol + 127) / 128), 3, 128, false, [&] { k_newton_assemble(ud, a); });
+  run_grid((unsigned)((ncol + 31) / 32), 1, 32 * kLuWarps, true, [&] { k_lu_factor(ud, lu.data(), ldw, ncol); });
+  run_grid((unsigned)((ncol + 127) / 128), 1, 128, false, [&] { k_lu_solve(ud, a); });
   return 0;
 }
 

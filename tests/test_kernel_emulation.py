@@ -18,8 +18,8 @@ from paper_2512_06729_b200 import binding
 EMU_DIR = os.path.join(ROOT, "tests", "kernel_emu")
 CSRC = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
 LIB = os.path.join(EMU_DIR, "libxod_emu.so")
-SOURCES = [os.path.join(EMU_DIR, "emu.cpp")] + [os.path.join(CSRC, f) for f in ("pack.cpp", "pack_fused.cpp", "pack_jac.cpp")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "jac_tiled.cuh", "sched.cuh", "xod_math.cuh", "xod_internal.h")] + [
+SOURCES = [os.path.join(EMU_DIR, "emu.cpp")] + [os.path.join(CSRC, f) for f in ("pack.cpp", "pack_fused.cpp", "pack_jac.cpp", "pack_lu.cpp")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "jac_tiled.cuh", "newton.cuh", "sched.cuh", "xod_math.cuh", "xod_internal.h")] + [
     os.path.join(EMU_DIR, "shim", "cuda_runtime.h"), os.path.join(EMU_DIR, "shim", "xod_cta.cuh")]
 
 
@@ -334,14 +334,23 @@ kf = np.abs(np.random.default_rng(1).normal(size=(net.n_reactions, atm.ld)))
 jac = np.zeros((binding_nnz(net), atm.ld))
 assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(atm.ld), tk.ptr(kf), tk.ptr(kf), tk.ptr(atm.n),
                               tk.ptr(jac), C.c_int(2), C.c_int(2)) == 0
+# the implicit step: k_lu_factor's shared row, one barrier per pivot
+net1 = synth.config_network(1)
+atm1 = synth.config_atmosphere(1, net1)
+d1, keep1 = tk.descriptor(net1)
+k1 = np.abs(np.random.default_rng(2).normal(size=(net1.n_reactions, atm1.ld))) * 1e-12
+y1 = atm1.n.copy()
+delta1 = np.zeros_like(y1)
+assert emu.emu_newton_step(C.byref(d1), C.c_int64(atm1.ncol), C.c_int64(atm1.ld), tk.ptr(k1), tk.ptr(k1), tk.ptr(atm1.n),
+                           tk.ptr(np.full(atm1.ld, 1e-3)), tk.ptr(y1), tk.ptr(delta1)) == 0
 print("emulated-ok")
 """
 
 
-def test_fused_and_tiled_jacobian_kernel_sources_are_race_free_under_thread_sanitizer():
+def test_barrier_synchronised_kernel_sources_are_race_free_under_thread_sanitizer():
     """racecheck substitute (compute-sanitizer is closed on the GPU pool): the emulated CUDA threads are
     real threads and __syncthreads a real barrier, so ThreadSanitizer sees every shared-memory access
-    of k_fused and k_jac_tiled between barriers: the double-buffered values and schedule, the accumulator
+    of k_fused, k_jac_tiled and k_lu_factor between barriers: the double-buffered values and schedule, the accumulator
     read-modify-writes of the row tasks, the per-unit flush, the tile prologue/epilogue.  (Removing the per-chunk barrier makes it report.)"""
     tsan = subprocess.run(["gcc", "-print-file-name=libtsan.so"], capture_output=True, text=True).stdout.strip()
     if not os.path.isabs(tsan) or not os.path.exists(tsan):
