@@ -199,3 +199,21 @@ class Oracle:
         if rc != 0:
             raise ArithmeticError("oracle Newton step failed (%d: -2 = singular matrix)" % rc)
         return delta, y_new
+
+    # ---- f2: photolysis rate constants
+    def photo_rates(self, ph, n, dz, j0, j_diff, mu, t_f, n_atm, n_layers, want_tau=False):
+        """k_ph [n_photo][ld] (and the layer-centre optical depths [n_bins][ld]).  `ph` is any object with
+        abs_species [n_abs], sigma_ext [n_abs][n_bins], sigma_ph [n_photo][n_bins], dlambda [n_bins]."""
+        n, dz, j0, mu, t_f = _f64(n), _f64(dz), _f64(j0), _f64(mu), _f64(t_f)
+        ld = n.shape[1]
+        sig_e, sig_p, dl = _f64(ph.sigma_ext), _f64(ph.sigma_ph), _f64(ph.dlambda)
+        ab = np.ascontiguousarray(ph.abs_species, dtype=np.int32)
+        nph, nb = sig_p.shape
+        jd = None if j_diff is None else _f64(j_diff)
+        kph = np.zeros((nph, ld))
+        tau = np.zeros((nb, ld)) if want_tau else None
+        rc = self.lib.orc_photo_rates(C.c_int(nph), C.c_int(nb), C.c_int(ab.shape[0]), _ptr(ab), _ptr(sig_e), _ptr(sig_p),
+                                      _ptr(dl), C.c_long(n_atm), C.c_long(n_layers), C.c_long(ld), _ptr(n), _ptr(dz), _ptr(j0),
+                                      _ptr(jd), _ptr(mu), _ptr(t_f), _ptr(kph), _ptr(tau))
+        assert rc == 0
+        return (kph, tau) if want_tau else kph

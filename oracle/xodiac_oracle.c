@@ -522,3 +522,53 @@ int orc_newton_step(const orc_network *net, long ncol, long ld, const double *kf
   free(A);
   return rc;
 }
+
+/* ---------------------------------------------------------------- f2: photolysis rate constants
+ * PAPER.md:165-213 (section 2.3.3).  For every atmosphere and wavelength bin:
+ *   optical depth   tau(z, lambda) = sum over the gas above z of (sigma_a,i + sigma_s,i) n_i dz
+ *   actinic flux    J(z, lambda) = J0(lambda) exp(-tau / mu) + J_diff(z, lambda)
+ *   rate constant   k_ph,i(z) = t_f * integral of J(z, lambda) sigma_i(lambda) d lambda
+ * Discretisation (readings H1-H4; the paper gives none): layers are columns
+ * a * n_layers + k with k = 0 at the bottom; tau is taken at the CENTRE of layer k, i.e. all layers above it
+ * plus half of its own; the integral is the rectangle rule over the bins, sum_b J sigma dlambda_b (the paper's
+ * bins are "approximately 1 A wide", uniform or not); J_diff = (J_up + J_down)/2 is an INPUT (the paper
+ * names no transfer scheme for it), NULL = 0; sigma_ext rows are sigma_a + sigma_s of the absorbing species
+ * abs_species[x]; sigma_ph rows are the reaction-specific cross-sections (molecular cross-section times
+ * quantum yield already applied), in the row order of the library's J input.
+ * Plain loops, one atmosphere and one bin at a time, top of the atmosphere downwards, in real_t.
+ * tau_out (optional) [n_bins][ld] receives the layer-centre optical depths.
+ * Pins (tests/test_oracle_photo.py): transparent atmosphere = t_f sum J0 sigma dlambda; a grey uniform slab
+ * against the closed form exp(-kappa (depth + dz/2) / mu); a one-bin cross-section; the invariance
+ * (sigma_ext, mu) -> (c sigma_ext, c mu); linearity in J0, sigma_ph and t_f; J_diff alone; monotone decrease downwards. */
+int orc_photo_rates(int n_photo, int n_bins, int n_abs, const int *abs_species, const double *sigma_ext,
+                    const double *sigma_ph, const double *dlambda, long n_atm, long n_layers, long ld,
+                    const double *n, const double *dz, const double *j0, const double *j_diff,
+                    const double *mu, const double *t_f, double *kph, double *tau_out) {
+  real_t *acc = (real_t *)malloc(sizeof(real_t) * (size_t)n_photo * (size_t)n_layers);
+  if (!acc) return -1;
+  for (long a = 0; a < n_atm; ++a) {
+    for (long e = 0; e < (long)n_photo * n_layers; ++e) acc[e] = 0;
+    for (int b = 0; b < n_bins; ++b) {
+      real_t above = 0; /* optical depth of everything above the current layer */
+      for (long k = n_layers - 1; k >= 0; --k) {
+        long c = a * n_layers + k;
+        real_t kappa = 0;
+        for (int x = 0; x < n_abs; ++x)
+          kappa += (real_t)sigma_ext[(long)x * n_bins + b] * (real_t)n[(long)abs_species[x] * ld + c];
+        real_t slab = kappa * (real_t)dz[c];
+        real_t tau = above + slab / 2;
+        above += slab;
+        if (tau_out) tau_out[(long)b * ld + c] = (double)tau;
+        real_t flux = (real_t)j0[a * n_bins + b] * R_EXP(-tau / (real_t)mu[a]);
+        if (j_diff) flux += (real_t)j_diff[(long)b * ld + c];
+        for (int p = 0; p < n_photo; ++p)
+          acc[(long)p * n_layers + k] += flux * (real_t)sigma_ph[(long)p * n_bins + b] * (real_t)dlambda[b];
+      }
+    }
+    for (int p = 0; p < n_photo; ++p)
+      for (long k = 0; k < n_layers; ++k)
+        kph[(long)p * ld + a * n_layers + k] = (double)((real_t)t_f[a] * acc[(long)p * n_layers + k]);
+  }
+  free(acc);
+  return 0;
+}

@@ -697,3 +697,77 @@ def edge_atmosphere(net, seed=2099, n_layers=75):
     atm.n[7, c + 4] = -atm.n[7, c + 4]
     atm.meta.update(cold=c, zero_species=5, zero_column=c + 2, negative=(7, c + 4))
     return atm
+
+
+# --------------------------------------------------------------------------- f2: photolysis inputs
+
+@dataclass
+class Photo:
+    """Wavelength grid and cross-sections for the photolysis rate constants."""
+    dlambda: np.ndarray       # float64 [n_bins]  bin widths, Angstrom
+    lam: np.ndarray           # float64 [n_bins]  bin centres, Angstrom (not used by the method; for plots/tests)
+    abs_species: np.ndarray   # int32 [n_abs]     species index of each extinction cross-section row
+    sigma_ext: np.ndarray     # float64 [n_abs][n_bins]    absorption + scattering, cm^2
+    sigma_ph: np.ndarray      # float64 [n_photo][n_bins]  cross-section of each photolysis reaction, cm^2
+
+    @property
+    def n_bins(self):
+        return int(self.dlambda.shape[0])
+
+
+def make_photo(seed, net, n_bins=10000, n_abs=None):
+    """Seeded stand-in for the PHIDRATES / Leiden cross-section tables, which are not in the container.
+    Shapes from the paper: bins about 1 A wide from 1 A to 10 000 A (10 000 of them; widths jittered
+    +-20 % so the grid is non-uniform, which the paper allows); every photolysis parent is an absorber plus a
+    few more species; a cross-section is a sum of one to three Gaussian bands (peak log-uniform 1e-20..1e-16
+    cm^2) over a Rayleigh-like lambda^-4 floor; a branch's cross-section is its parent's absorption times a
+    quantum yield that is smooth in wavelength and vanishes above a threshold."""
+    rng = np.random.default_rng(seed)
+    dl = (10000.0 - 1.0) / n_bins * rng.uniform(0.8, 1.2, size=n_bins)
+    dl *= (10000.0 - 1.0) / dl.sum()
+    edges = 1.0 + np.concatenate([[0.0], np.cumsum(dl)])
+    lam = 0.5 * (edges[:-1] + edges[1:])
+    photo_rows = np.flatnonzero(net.type == PHOTO)
+    parents = net.reactants[photo_rows, 0]
+    others = rng.permutation(np.setdiff1d(np.arange(net.n_species), parents))
+    extra = others[:max(0, (n_abs or (len(np.unique(parents)) + 8)) - len(np.unique(parents)))]
+    abs_species = np.concatenate([np.unique(parents), np.sort(extra)]).astype(np.int32)
+
+    def bands():
+        s = 1e-26 * (lam / 1000.0) ** -4.0
+        for _ in range(rng.integers(1, 4)):
+            s = s + _loguniform(rng, 1e-20, 1e-16) * np.exp(-0.5 * ((lam - rng.uniform(300.0, 4000.0)) / rng.uniform(50.0, 1500.0)) ** 2)
+        return s
+
+    sigma_ext = np.stack([bands() for _ in abs_species])
+    row_of = {int(sp): k for k, sp in enumerate(abs_species)}
+    sigma_ph = np.zeros((len(photo_rows), n_bins))
+    for p, parent in enumerate(parents):
+        threshold = rng.uniform(1500.0, 6000.0)
+        yield_ = rng.uniform(0.05, 1.0) / (1.0 + np.exp((lam - threshold) / rng.uniform(20.0, 200.0)))
+        sigma_ph[p] = sigma_ext[row_of[int(parent)]] * yield_
+    return Photo(dlambda=dl, lam=lam, abs_species=abs_species, sigma_ext=sigma_ext, sigma_ph=sigma_ph)
+
+
+def make_irradiation(seed, net, atm, photo, with_diffuse=True):
+    """Per-atmosphere irradiation for `make_photo`: layer thickness dz [ld] (cm) from the hydrostatic spacing of
+    the log-pressure grid, stellar photon flux at the top j0 [n_atm][n_bins] (a Planck-like photon spectrum of
+    4 000-7 000 K scaled to 1e10..1e14 photons cm^-2 s^-1 A^-1 at its peak), a diffuse term j_diff [n_bins][ld] of a
+    few per cent of it, the cosine of the zenith angle mu [n_atm] in 0.3..1 and the irradiated-time fraction
+    t_f [n_atm] in {1, 1/2} (PAPER.md:213)."""
+    rng = np.random.default_rng(seed)
+    n_atm, L = atm.meta["n_atm"], atm.meta["n_layers"]
+    dz = np.ones(atm.ld)
+    dlnp = np.log(1.0e11) / max(L - 1, 1)
+    dz[:atm.ncol] = dlnp * K_B * atm.T[:atm.ncol] / (2.3 * 1.6726e-24 * 2000.0)
+    x = 1.4388e8 / (photo.lam[None, :] * rng.uniform(4000.0, 7000.0, size=(n_atm, 1)))      # h c / (lambda k_B T)
+    shape = photo.lam[None, :] ** -4.0 / np.expm1(np.minimum(x, 700.0))
+    j0 = shape / shape.max(axis=1, keepdims=True) * _loguniform(rng, 1e10, 1e14, size=(n_atm, 1))
+    mu = rng.uniform(0.3, 1.0, size=n_atm)
+    t_f = rng.choice([1.0, 0.5], size=n_atm)
+    j_diff = None
+    if with_diffuse:
+        j_diff = np.zeros((photo.n_bins, atm.ld))
+        for a in range(n_atm):
+            j_diff[:, a * L:(a + 1) * L] = j0[a][:, None] * rng.uniform(0.0, 0.05, size=(photo.n_bins, L))
+    return dz, j0, j_diff, mu, t_f
