@@ -327,6 +327,67 @@ def stage_timings(binding, h3, net, dev, ws_for, dfma_per_s):
             del jac
         out["config%d" % cfg] = res
         del kf, kr, d, th
+    out.update(next_row_timings(binding, net, dev, ws_for))
+    return out
+
+
+def next_row_timings(binding, net, dev, ws_for):
+    """Device times of the SURVEY section 8(f) rows that are built: f1 (one Newton iteration of the backward-Euler step,
+    2 048 columns of config 5 = one workspace pass) and f2 (photolysis rate constants, 10 000 bins, 8 atmospheres)."""
+    import torch
+    from paper_2512_06729_b200 import synth
+    out = {}
+    sync = torch.cuda.synchronize
+    try:
+        atm = synth.make_atmosphere(2005, net, 14, 150)                      # 2 100 columns, the first 2 048 used
+        ncol, ld, ns, nr = 2048, atm.ld, net.n_species, net.n_reactions
+        h = binding.Network(net, device=torch.cuda.current_device(), flags=binding.XOD_FLAG_BUILD_LU)
+        T, P, J, n = dev(atm.T), dev(atm.P), dev(atm.J), dev(atm.n)
+        kf = torch.empty((nr, ld), dtype=torch.float64, device="cuda")
+        kr = torch.empty_like(kf)
+        h.rate_coeffs(ncol, ld, T, P, J, kf, kr, ws_for(h.rate_coeffs_workspace_bytes(ncol)))
+        dt = torch.full((ld,), 1.0e-9, dtype=torch.float64, device="cuda")
+        ws = ws_for(h.newton_workspace_bytes(ncol))
+        y = n.clone()
+        step = lambda: h.newton_step(ncol, ld, kf, kr, n, dt, y, None, workspace=ws)
+        step()
+        sync()
+        h.tune(binding.XOD_TUNE_TIMING, 1)
+        ms = event_time_ms(step, 2, sync)
+        kt = h.timing_read()
+        h.tune(binding.XOD_TUNE_TIMING, 0)
+        info = h.lu_info()
+        out["f1_newton_step"] = {"ncol": ncol, "ms": ms, "columns_per_s": ncol / (ms * 1e-3),
+                                 "kernel_ms": {k: v[0] / 2 for k, v in kt.items() if v[1]},
+                                 "nnz_lu": info["nnz_lu"], "updates_per_column": info["updates"],
+                                 "factor_gflops": 2e-9 * info["updates"] * ncol / (kt["lu_factor"][0] / 2 * 1e-3) if kt["lu_factor"][1] else None}
+        del ws, kf, kr, y
+        h.close()
+    except Exception as exc:
+        out["f1_newton_step"] = {"error": repr(exc)[:300]}
+    try:
+        atm = synth.make_atmosphere(2005, net, 8, 150)
+        ph = synth.make_photo(31, net, n_bins=10000)
+        dz, j0, jd, mu, tf = synth.make_irradiation(32, net, atm, ph, with_diffuse=False)
+        h = binding.Network(net, device=torch.cuda.current_device())
+        p = binding.Photo(h, ph)
+        Jout = torch.empty((net.n_photo, atm.ld), dtype=torch.float64, device="cuda")
+        ws = ws_for(p.workspace_bytes(atm.ncol))
+        args = (8, 150, atm.ld, dev(atm.n), dev(dz), dev(j0), None, dev(mu), dev(tf), Jout, ws)
+        call = lambda: p.rates(*args)
+        call()
+        sync()
+        h.tune(binding.XOD_TUNE_TIMING, 1)
+        ms = event_time_ms(call, 3, sync)
+        kt = h.timing_read()
+        h.tune(binding.XOD_TUNE_TIMING, 0)
+        flop = 2.0 * ph.n_bins * (net.n_photo + len(ph.abs_species)) * atm.ncol
+        out["f2_photo_rates"] = {"ncol": atm.ncol, "n_bins": ph.n_bins, "ms": ms, "tflops": flop / (ms * 1e-3) / 1e12,
+                                 "kernel_ms": {k: v[0] / 3 for k, v in kt.items() if v[1]}}
+        p.close()
+        h.close()
+    except Exception as exc:
+        out["f2_photo_rates"] = {"error": repr(exc)[:300]}
     return out
 
 

@@ -149,7 +149,8 @@ xod_status xod_network_tune(xod_network *net, int32_t knob, int64_t value);
 enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD_KERNEL_RATES_FROM_K = 3,
        XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
        XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_JAC_TILED = 9, XOD_KERNEL_NEWTON_ASSEMBLE = 10,
-       XOD_KERNEL_LU_FACTOR = 11, XOD_KERNEL_LU_SOLVE = 12, XOD_KERNEL_COUNT = 13 };
+       XOD_KERNEL_LU_FACTOR = 11, XOD_KERNEL_LU_SOLVE = 12, XOD_KERNEL_PHOTO_GEMM = 13, XOD_KERNEL_PHOTO_FLUX = 14,
+       XOD_KERNEL_COUNT = 15 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);
@@ -226,6 +227,39 @@ size_t xod_newton_workspace_bytes(const xod_network *net, int64_t ncol);
 xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,
                            const double *n_old, const double *dt, double *y, double *delta, void *workspace,
                            size_t workspace_bytes, void *stream);
+
+/* ---- f2: photolysis rate constants, the J input of the calls above.
+ *   tau(z, lambda) = sum over the gas above z of (sigma_a,i + sigma_s,i) n_i dz
+ *   J(z, lambda)   = J0(lambda) exp(-tau / mu) + J_diff(z, lambda)
+ *   k_ph,i(z)      = t_f * integral J(z, lambda) sigma_i(lambda) d lambda
+ * Discretisation (readings H1-H4): column = atmosphere * n_layers + layer, layer 0 at the bottom;
+ * tau at the CENTRE of a layer (everything above it plus half of its own kappa dz); rectangle rule over the
+ * wavelength bins, sum_b J sigma dlambda_b (uniform or non-uniform widths); J_diff = (J_up + J_down)/2
+ * is an input (NULL = 0).  t_f is the irradiated-time fraction.
+ * xod_photo_desc (HOST pointers, copied): dlambda [n_bins] bin widths; abs_species [n_abs] species index of each
+ * extinction row; sigma_ext [n_abs][n_bins] = sigma_a + sigma_s in cm^2; sigma_ph [n_photo][n_bins] = the
+ * reaction-specific cross-section (PHIDRATES kind, or molecular cross-section times quantum yield)
+ * of the p-th XOD_PHOTO reaction in user order, i.e. row p of J.  All values finite and >= 0.
+ * xod_photo_rates: n [n_species][ld], dz [ld] layer thickness in cm, j0 [n_atm][n_bins] photons cm^-2 s^-1 per unit
+ * of dlambda at the top of the atmosphere, j_diff [n_bins][ld] or NULL, mu [n_atm] cosine of the zenith angle (> 0),
+ * t_f [n_atm], J [n_photo][ld] out: device memory owned by the caller; columns >= n_atm * n_layers are not touched;
+ * workspace >= xod_photo_workspace_bytes(photo, n_atm * n_layers) (one [n_bins][columns] array).
+ * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, n_layers > 907, n_atm > 65535), XOD_ERR_WORKSPACE, XOD_ERR_CUDA.
+ * The photo object keeps a pointer to `net`: destroy it before the network. */
+typedef struct xod_photo xod_photo;
+typedef struct {
+  int32_t n_bins, n_abs;
+  const double *dlambda;
+  const int32_t *abs_species;
+  const double *sigma_ext;
+  const double *sigma_ph;
+} xod_photo_desc;
+xod_status xod_photo_create(const xod_network *net, const xod_photo_desc *desc, xod_photo **out);
+void xod_photo_destroy(xod_photo *photo);
+size_t xod_photo_workspace_bytes(const xod_photo *photo, int64_t ncol);
+xod_status xod_photo_rates(const xod_photo *photo, int64_t n_atm, int64_t n_layers, int64_t ld, const double *n,
+                           const double *dz, const double *j0, const double *j_diff, const double *mu,
+                           const double *t_f, double *J, void *workspace, size_t workspace_bytes, void *stream);
 
 /* ---- end-to-end convenience: the fused call on HOST buffers (pinned for overlap; pageable works
  * but serialises).  Columns are processed in chunks of one round of tiles per SM through three

@@ -17,7 +17,7 @@ XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK, XOD_FLAG_BUILD_LU = 1, 2
 XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL, XOD_TUNE_JAC_TILED = 0, 1, 2, 3, 4
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve"]
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve", "photo_gemm", "photo_flux"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -28,7 +28,8 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_source", "xod_source_fused_workspace_bytes", "xod_source_fused", "xod_jacobian",
            "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params",
            "xod_check_status", "xod_build_has_checks", "xod_network_jac_info", "xod_network_lu_info", "xod_network_lu_pattern",
-           "xod_newton_workspace_bytes", "xod_newton_step"]
+           "xod_newton_workspace_bytes", "xod_newton_step", "xod_photo_create", "xod_photo_destroy",
+           "xod_photo_workspace_bytes", "xod_photo_rates"]
 
 
 class XodError(RuntimeError):
@@ -59,6 +60,10 @@ def lib():
                      "xod_source_fused_workspace_bytes", "xod_newton_workspace_bytes"):
             getattr(L, name).restype = C.c_size_t
             getattr(L, name).argtypes = [C.c_void_p, C.c_int64]
+        L.xod_photo_workspace_bytes.restype = C.c_size_t
+        L.xod_photo_workspace_bytes.argtypes = [C.c_void_p, C.c_int64]
+        L.xod_photo_destroy.restype = None
+        L.xod_photo_destroy.argtypes = [C.c_void_p]
         L.xod_launch_count.restype = C.c_int64
         L.xod_network_destroy.restype = None
         L.xod_network_destroy.argtypes = [C.c_void_p]
@@ -260,6 +265,40 @@ class Network:
             return C.c_void_p(a.data_ptr())
         _check(lib().xod_source_fused_host(self._h, C.c_int64(ncol), C.c_int64(ld), hp(T), hp(P), hp(J),
                                            hp(n), hp(dndt)))
+
+
+class _PhotoDesc(C.Structure):
+    _fields_ = [("n_bins", C.c_int32), ("n_abs", C.c_int32), ("dlambda", C.c_void_p), ("abs_species", C.c_void_p),
+                ("sigma_ext", C.c_void_p), ("sigma_ph", C.c_void_p)]
+
+
+class Photo:
+    """xod_photo handle (f2).  `ph` is any object with dlambda, abs_species, sigma_ext, sigma_ph (synth.Photo)."""
+
+    def __init__(self, network, ph):
+        keep = dict(dlambda=_np(ph.dlambda, np.float64), abs_species=_np(ph.abs_species, np.int32),
+                    sigma_ext=_np(ph.sigma_ext, np.float64), sigma_ph=_np(ph.sigma_ph, np.float64))
+        d = _PhotoDesc(keep["dlambda"].shape[0], keep["abs_species"].shape[0],
+                       *[_hp(keep[k]) for k in ("dlambda", "abs_species", "sigma_ext", "sigma_ph")])
+        h = C.c_void_p()
+        _check(lib().xod_photo_create(network._h, C.byref(d), C.byref(h)))
+        self._h, self._net = h, network          # the photo object points into the network: keep it alive
+        self.n_bins = d.n_bins
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().xod_photo_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def workspace_bytes(self, ncol):
+        return lib().xod_photo_workspace_bytes(self._h, ncol)
+
+    def rates(self, n_atm, n_layers, ld, n, dz, j0, j_diff, mu, t_f, J, workspace, stream=None):
+        _check(lib().xod_photo_rates(self._h, C.c_int64(n_atm), C.c_int64(n_layers), C.c_int64(ld), _dp(n), _dp(dz), _dp(j0),
+                                     _dp(j_diff), _dp(mu), _dp(t_f), _dp(J), _dp(workspace),
+                                     C.c_size_t(0 if workspace is None else workspace.numel() * 8), _stream(stream)))
 
 
 def build_has_checks():

@@ -10,6 +10,7 @@
 #include "fused.cuh"
 #include "jac_tiled.cuh"
 #include "newton.cuh"
+#include "photo.cuh"
 #include "rates2.cuh"
 #include "kernels.cuh"
 
@@ -881,6 +882,121 @@ xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, con
       k_lu_solve<<<(unsigned)((w + 127) / 128), 128, 0, s>>>(net->ld, a);
       XOD_CUDA(cudaGetLastError());
     }
+  }
+  return XOD_OK;
+}
+
+// ---------------------------------------------------------------------------- f2: photolysis rate constants
+
+xod_status xod_photo_create(const xod_network *net, const xod_photo_desc *d, xod_photo **out) {
+  if (!out) return fail(XOD_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (!net || !d) return fail(XOD_ERR_INVALID_ARG, "net or desc is NULL");
+  if (d->n_bins <= 0 || d->n_abs < 0) return fail(XOD_ERR_INVALID_ARG, "n_bins must be > 0 and n_abs >= 0");
+  if (!d->dlambda || (net->h.n_photo > 0 && !d->sigma_ph) || (d->n_abs > 0 && (!d->abs_species || !d->sigma_ext)))
+    return fail(XOD_ERR_INVALID_ARG, "dlambda, sigma_ph, abs_species, sigma_ext must not be NULL");
+  for (int x = 0; x < d->n_abs; ++x)
+    if (d->abs_species[x] < 0 || d->abs_species[x] >= net->h.ns) return fail(XOD_ERR_INVALID_ARG, "abs_species index out of range");
+  const size_t nb = (size_t)d->n_bins;
+  auto all_ok = [](const double *p, size_t n) {
+    for (size_t i = 0; i < n; ++i)
+      if (!std::isfinite(p[i]) || p[i] < 0) return false;
+    return true;
+  };
+  if (!all_ok(d->dlambda, nb) || !all_ok(d->sigma_ext, nb * d->n_abs) || !all_ok(d->sigma_ph, nb * net->h.n_photo))
+    return fail(XOD_ERR_INVALID_ARG, "bin widths and cross-sections must be finite and >= 0");
+  xod_photo *ph = new (std::nothrow) xod_photo;
+  if (!ph) return fail(XOD_ERR_ALLOC, "out of host memory");
+  ph->net = net, ph->device = net->device, ph->n_bins = d->n_bins, ph->n_abs = d->n_abs, ph->n_photo = net->h.n_photo;
+  ph->h_dlambda.assign(d->dlambda, d->dlambda + nb);
+  ph->h_sigma_ext.assign(d->sigma_ext, d->sigma_ext + nb * d->n_abs);
+  ph->h_sigma_ph.assign(d->sigma_ph, d->sigma_ph + nb * net->h.n_photo);
+  ph->h_abs.assign(d->abs_species, d->abs_species + d->n_abs);
+  if (ph->device >= 0) {
+    DeviceGuard guard(ph->device);
+    cudaError_t e = guard.err;
+    auto up = [&](const void *src, size_t bytes, void **dst) {
+      if (e != cudaSuccess) return;
+      e = cudaMalloc(dst, std::max<size_t>(bytes, 16));
+      if (e == cudaSuccess && bytes) e = cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice);
+    };
+    up(ph->h_dlambda.data(), nb * 8, (void **)&ph->dlambda);
+    up(ph->h_sigma_ext.data(), ph->h_sigma_ext.size() * 8, (void **)&ph->sigma_ext);
+    up(ph->h_sigma_ph.data(), ph->h_sigma_ph.size() * 8, (void **)&ph->sigma_ph);
+    up(ph->h_abs.data(), ph->h_abs.size() * 4, (void **)&ph->abs_species);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_photo_flux, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
+    if (e != cudaSuccess) {
+      xod_photo_destroy(ph);
+      return cuda_fail(e, "xod_photo_create");
+    }
+  }
+  *out = ph;
+  return XOD_OK;
+}
+
+void xod_photo_destroy(xod_photo *ph) {
+  if (!ph) return;
+  if (ph->dlambda) cudaFree(ph->dlambda);
+  if (ph->sigma_ext) cudaFree(ph->sigma_ext);
+  if (ph->sigma_ph) cudaFree(ph->sigma_ph);
+  if (ph->abs_species) cudaFree(ph->abs_species);
+  delete ph;
+}
+
+size_t xod_photo_workspace_bytes(const xod_photo *ph, int64_t ncol) {
+  if (!ph || ncol < 0) return 0;
+  return (size_t)ph->n_bins * (size_t)round_up(std::max<int64_t>(ncol, 1), 32) * sizeof(double) + 256;
+}
+
+xod_status xod_photo_rates(const xod_photo *ph, int64_t n_atm, int64_t n_layers, int64_t ld, const double *n,
+                           const double *dz, const double *j0, const double *j_diff, const double *mu,
+                           const double *t_f, double *J, void *workspace, size_t workspace_bytes, void *stream) {
+  if (!ph) return fail(XOD_ERR_INVALID_ARG, "photo is NULL");
+  if (n_atm < 0 || n_layers < 0) return fail(XOD_ERR_INVALID_ARG, "n_atm or n_layers < 0");
+  const int64_t ncol = n_atm * n_layers;
+  xod_status st = check_common(ph->net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0 || ph->n_photo == 0) return XOD_OK;
+  if (!n || !dz || !j0 || !mu || !t_f || !J) return fail(XOD_ERR_INVALID_ARG, "n, dz, j0, mu, t_f or J is NULL");
+  if (!workspace || workspace_bytes < xod_photo_workspace_bytes(ph, ncol))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_photo_workspace_bytes");
+  const size_t smem = (size_t)32 * (size_t)(n_layers | 1) * sizeof(double);
+  if (smem > kFusedSmemMax) return fail(XOD_ERR_INVALID_ARG, "n_layers too large for one call (max 907)");
+  if (n_atm > 65535) return fail(XOD_ERR_INVALID_ARG, "n_atm too large for one call (max 65535)");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const xod_network *net = ph->net;
+  const int64_t ldw = round_up(ncol, 32);
+  double *F = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
+  {   // kappa[b][col] = sum_x sigma_ext[x][b] n[abs_species[x]][col]
+    GemmArgs g{};
+    g.M = ph->n_bins, g.N = ncol, g.K = ph->n_abs;
+    g.A = ph->sigma_ext, g.lda = ph->n_bins;
+    g.B = n, g.brow = ph->abs_species, g.ldb = ld, g.n_brows = net->h.ns;
+    g.C = F, g.ldc = ldw, g.scale_atm = nullptr, g.n_layers = 1;
+    dim3 grid((unsigned)((ncol + kGemmBN - 1) / kGemmBN), (unsigned)((ph->n_bins + kGemmBM - 1) / kGemmBM));
+    Timed tm(net, KID_PHOTO_GEMM, s);
+    k_photo_gemm<false><<<grid, 256, 0, s>>>(g);
+    XOD_CUDA(cudaGetLastError());
+  }
+  {   // tau (layer centres, top down), Beer-Lambert, times the bin width, in place
+    FluxArgs f{};
+    f.n_bins = ph->n_bins, f.n_atm = n_atm, f.n_layers = n_layers, f.ld = ld, f.ldw = ldw;
+    f.F = F, f.dz = dz, f.j0 = j0, f.j_diff = j_diff, f.mu = mu, f.dlambda = ph->dlambda;
+    dim3 grid((unsigned)((ph->n_bins + 31) / 32), (unsigned)n_atm);
+    Timed tm(net, KID_PHOTO_FLUX, s);
+    k_photo_flux<<<grid, 256, smem, s>>>(f);
+    XOD_CUDA(cudaGetLastError());
+  }
+  {   // J[p][col] = t_f sum_b sigma_ph[p][b] F[b][col]
+    GemmArgs g{};
+    g.M = ph->n_photo, g.N = ncol, g.K = ph->n_bins;
+    g.A = ph->sigma_ph, g.lda = ph->n_bins;
+    g.B = F, g.brow = nullptr, g.ldb = ldw, g.n_brows = ph->n_bins;
+    g.C = J, g.ldc = ld, g.scale_atm = t_f, g.n_layers = n_layers;
+    dim3 grid((unsigned)((ncol + kGemmBN - 1) / kGemmBN), (unsigned)((ph->n_photo + kGemmBM - 1) / kGemmBM));
+    Timed tm(net, KID_PHOTO_GEMM, s);
+    k_photo_gemm<true><<<grid, 256, 0, s>>>(g);
+    XOD_CUDA(cudaGetLastError());
   }
   return XOD_OK;
 }

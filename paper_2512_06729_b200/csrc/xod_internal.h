@@ -214,7 +214,7 @@ size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused
@@ -222,6 +222,17 @@ struct TimingState {
   std::vector<int> kid;                           // kernel id of pair p = events 2p, 2p+1
 };
 }  // namespace xod
+
+// f2: wavelength grid and cross-sections on the device (xod_photo_create)
+struct xod_photo {
+  const xod_network *net = nullptr;
+  int device = -1;
+  int32_t n_bins = 0, n_abs = 0, n_photo = 0;
+  std::vector<double> h_dlambda, h_sigma_ext, h_sigma_ph;
+  std::vector<int32_t> h_abs;
+  double *dlambda = nullptr, *sigma_ext = nullptr, *sigma_ph = nullptr;
+  int32_t *abs_species = nullptr;
+};
 
 constexpr int kHostSlots = 3;  // staging slots of xod_source_fused_host
 

@@ -19,6 +19,7 @@ void emu_syncthreads() { g_barrier->arrive_and_wait(); }
 #include "../../paper_2512_06729_b200/csrc/rates2.cuh"
 #include "../../paper_2512_06729_b200/csrc/jac_tiled.cuh"
 #include "../../paper_2512_06729_b200/csrc/newton.cuh"
+#include "../../paper_2512_06729_b200/csrc/photo.cuh"
 #include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
@@ -251,6 +252,38 @@ int emu_newton_step(const xod_network_desc *desc, int64_t ncol, int64_t ld, cons
   run_grid((unsigned)((ncol + 127) / 128), 3, 128, false, [&] { k_newton_assemble(ud, a); });
   run_grid((unsigned)((ncol + 31) / 32), 1, 32 * kLuWarps, true, [&] { k_lu_factor(ud, lu.data(), ldw, ncol); });
   run_grid((unsigned)((ncol + 127) / 128), 1, 128, false, [&] { k_lu_solve(ud, a); });
+  return 0;
+}
+
+// f2: photolysis rate constants, composed as xod_photo_rates composes them: k_photo_gemm (kappa), k_photo_flux,
+// k_photo_gemm (quadrature)
+int emu_photo_rates(int ns, int n_photo, int n_bins, int n_abs, const int32_t *abs_species, const double *sigma_ext,
+                    const double *sigma_ph, const double *dlambda, int64_t n_atm, int64_t n_layers, int64_t ld,
+                    const double *n, const double *dz, const double *j0, const double *j_diff, const double *mu,
+                    const double *t_f, double *J) {
+  const int64_t ncol = n_atm * n_layers, ldw = (ncol + 31) / 32 * 32;
+  if (ncol <= 0 || (size_t)32 * (n_layers | 1) * 8 > sizeof(smem_raw)) return 1;
+  std::vector<double> F((size_t)n_bins * ldw, NAN);
+  {
+    GemmArgs g{};
+    g.M = n_bins, g.N = ncol, g.K = n_abs, g.A = sigma_ext, g.lda = n_bins, g.B = n, g.brow = abs_species, g.ldb = ld;
+    g.n_brows = ns, g.C = F.data(), g.ldc = ldw, g.scale_atm = nullptr, g.n_layers = 1;
+    run_grid((unsigned)((ncol + kGemmBN - 1) / kGemmBN), (unsigned)((n_bins + kGemmBM - 1) / kGemmBM), 256, true,
+             [&] { k_photo_gemm<false>(g); });
+  }
+  {
+    FluxArgs f{};
+    f.n_bins = n_bins, f.n_atm = n_atm, f.n_layers = n_layers, f.ld = ld, f.ldw = ldw;
+    f.F = F.data(), f.dz = dz, f.j0 = j0, f.j_diff = j_diff, f.mu = mu, f.dlambda = dlambda;
+    run_grid((unsigned)((n_bins + 31) / 32), (unsigned)n_atm, 256, true, [&] { k_photo_flux(f); });
+  }
+  {
+    GemmArgs g{};
+    g.M = n_photo, g.N = ncol, g.K = n_bins, g.A = sigma_ph, g.lda = n_bins, g.B = F.data(), g.brow = nullptr, g.ldb = ldw;
+    g.n_brows = n_bins, g.C = J, g.ldc = ld, g.scale_atm = t_f, g.n_layers = n_layers;
+    run_grid((unsigned)((ncol + kGemmBN - 1) / kGemmBN), (unsigned)((n_photo + kGemmBM - 1) / kGemmBM), 256, true,
+             [&] { k_photo_gemm<true>(g); });
+  }
   return 0;
 }
 
