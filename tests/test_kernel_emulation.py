@@ -77,6 +77,21 @@ def test_fused_kernel_source_matches_oracle(emu, oracle, network, cfg, grid, nsp
     check(got, want, wp + wl, atm.ncol, "emulated k_fused config %d" % cfg)
 
 
+def test_fused_kernel_source_on_the_594_species_network(emu, oracle, network):
+    """The production network (config 3: 33 chunks of 240 reactions, 609 accumulator rows with hub-species extras,
+    227 KB of shared memory) on 20 columns = one full and one ragged tile, chunks split 3 ways, fewer blocks than
+    work items -- the launch shape of the few-column path."""
+    from paper_2512_06729_b200 import synth
+    net = network(3)
+    atm = synth.make_atmosphere(2033, net, 1, 20)
+    want, wp, wl = oracle.source_from_state(net, atm.T, atm.P, atm.J, atm.n, atm.ncol)
+    got = run_fused(emu, net, atm, atm.ncol, grid=4, nsplit=3)
+    check(got, want, wp + wl, atm.ncol, "emulated k_fused config 3")
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, atm.ncol)
+    got_k = run_fused(emu, net, atm, atm.ncol, kf=np.ascontiguousarray(okf), kr=np.ascontiguousarray(okr), grid=2, nsplit=1)
+    check(got_k, want, wp + wl, atm.ncol, "emulated k_fused<FROMK> config 3")
+
+
 def test_fused_kernel_source_from_stored_coefficients_and_mixed_intervals(emu, oracle, network):
     """k_fused<true> (xod_source), and a tile whose columns straddle thermo breakpoints (the rare
     per-thread second parameter block) with cold columns whose k_r overflow."""
@@ -341,10 +356,69 @@ d1, keep1 = tk.descriptor(net1)
 k1 = np.abs(np.random.default_rng(2).normal(size=(net1.n_reactions, atm1.ld))) * 1e-12
 y1 = atm1.n.copy()
 delta1 = np.zeros_like(y1)
+dt1 = np.full(atm1.ld, 1e-3)
 assert emu.emu_newton_step(C.byref(d1), C.c_int64(atm1.ncol), C.c_int64(atm1.ld), tk.ptr(k1), tk.ptr(k1), tk.ptr(atm1.n),
-                           tk.ptr(np.full(atm1.ld, 1e-3)), tk.ptr(y1), tk.ptr(delta1)) == 0
+                           tk.ptr(dt1), tk.ptr(y1), tk.ptr(delta1)) == 0
 print("emulated-ok")
 """
+
+
+ASAN_CHILD = r"""
+import sys, ctypes as C
+sys.path.insert(0, sys.argv[1]); sys.path.insert(0, sys.argv[1] + "/tests")
+import numpy as np
+import test_kernel_emulation as tk
+import test_photo_rates as tp
+from paper_2512_06729_b200 import synth, binding
+emu = C.CDLL(sys.argv[2])
+tk.LIB = tp_lib = sys.argv[2]
+# exact-size heap buffers (numpy) around every kernel: any access outside [0, rows x ld) is reported
+for net, atm in ((synth.config_network(2), None), (synth.edge_network(), None)):
+    atm = synth.edge_atmosphere(net) if net.meta.get("name") == "edge" else synth.config_atmosphere(2, net)
+    ncol = atm.ncol - 3                                   # ragged: the last tile and the last warp are partial
+    tk.run_fused(emu, net, atm, ncol, grid=3, nsplit=2)
+    d, keep = tk.descriptor(net)
+    nr, ns, ld = net.n_reactions, net.n_species, atm.ld
+    kf, kr = np.full((nr, ld), 1e-12), np.full((nr, ld), 1e-13)
+    assert emu.emu_rate_coeffs(C.byref(d), C.c_int64(ncol), C.c_int64(ld), tk.ptr(atm.T), tk.ptr(atm.P), tk.ptr(atm.J),
+                               tk.ptr(kf), tk.ptr(kr), C.c_int(12)) == 0
+    kr[~np.isfinite(kr)] = 0.0
+    tk.run_fused(emu, net, atm, ncol, kf=kf, kr=kr, grid=2, nsplit=1)
+    nnz = binding.Network(net, device=-1).nnz_jac
+    jac = np.zeros((nnz, ld))
+    assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), tk.ptr(kf), tk.ptr(kr), tk.ptr(atm.n), tk.ptr(jac),
+                                  C.c_int(2), C.c_int(3)) == 0
+    assert emu.emu_jacobian(C.byref(d), C.c_int64(ncol), C.c_int64(ld), tk.ptr(kf), tk.ptr(kr), tk.ptr(atm.n), tk.ptr(jac), C.c_int(3)) == 0
+    dn, pr, lo = (np.zeros((ns, ld)) for _ in range(3))
+    assert emu.emu_source_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), tk.ptr(atm.T), tk.ptr(atm.P), tk.ptr(atm.J),
+                                   None, None, tk.ptr(atm.n), tk.ptr(dn), tk.ptr(pr), tk.ptr(lo), C.c_int(16)) == 0
+    y, delta, n_old, dt = np.abs(atm.n).copy(), np.zeros((ns, ld)), np.abs(atm.n).copy(), np.full(ld, 1e-9)
+    assert emu.emu_newton_step(C.byref(d), C.c_int64(min(ncol, 37)), C.c_int64(ld), tk.ptr(kf), tk.ptr(kr), tk.ptr(n_old),
+                               tk.ptr(dt), tk.ptr(y), tk.ptr(delta)) == 0
+net = synth.config_network(1)
+atm = synth.config_atmosphere(1, net, 3)
+ph = synth.make_photo(51, net, n_bins=70)
+tp.run_emulated(net, atm, ph, *synth.make_irradiation(52, net, atm, ph))
+print("emulated-ok")
+"""
+
+
+def test_kernel_sources_touch_no_memory_outside_their_buffers_under_address_sanitizer():
+    """memcheck substitute (compute-sanitizer is closed on the GPU pool): the emulation built with AddressSanitizer
+    and UndefinedBehaviorSanitizer (alignment, bounds, shifts), every kernel run on exact-size heap buffers with ragged
+    column counts: an access one element past a [rows][ld] array, a misaligned 16-byte vector access or an index
+    beyond a static shared array aborts the child."""
+    asan = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(asan) or not os.path.exists(asan):
+        pytest.skip("libasan not available")
+    lib = os.path.join(EMU_DIR, "libxod_emu_asan.so")
+    if not os.path.exists(lib) or any(os.path.getmtime(d) > os.path.getmtime(lib) for d in DEPS):
+        subprocess.run(["g++", "-std=c++20", "-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                        "-pthread", "-shared", "-fPIC", "-I" + os.path.join(EMU_DIR, "shim"), "-o", lib] + SOURCES, check=True)
+    env = dict(os.environ, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:halt_on_error=1", UBSAN_OPTIONS="print_stacktrace=1")
+    out = subprocess.run([os.sys.executable, "-c", ASAN_CHILD, ROOT, lib], capture_output=True, text=True, env=env, timeout=1800)
+    assert "emulated-ok" in out.stdout, (out.stdout[-1000:], out.stderr[-3000:])
+    assert "AddressSanitizer" not in out.stderr and "runtime error" not in out.stderr, out.stderr[-3000:]
 
 
 def test_barrier_synchronised_kernel_sources_are_race_free_under_thread_sanitizer():
