@@ -217,3 +217,16 @@ class Oracle:
                                       _ptr(jd), _ptr(mu), _ptr(t_f), _ptr(kph), _ptr(tau))
         assert rc == 0
         return (kph, tau) if want_tau else kph
+
+    # ---- f3: molecular-diffusion transport terms (Eq. 3-4)
+    def transport(self, n, T, n_gas, D, mass, alpha_T, mbar, grav, dz, n_atm, n_layers, want_d=False):
+        """tr [n_species][ld] (and d_{k+1/2} [n_species][ld])."""
+        n, T, n_gas, D = _f64(n), _f64(T), _f64(n_gas), _f64(D)
+        mass, alpha_T, mbar, grav, dz = _f64(mass), _f64(alpha_T), _f64(mbar), _f64(grav), _f64(dz)
+        ns, ld = n.shape
+        tr = np.zeros((ns, ld))
+        d = np.zeros((ns, ld)) if want_d else None
+        rc = self.lib.orc_transport(C.c_int(ns), C.c_long(n_atm), C.c_long(n_layers), C.c_long(ld), _ptr(n), _ptr(T), _ptr(n_gas),
+                                    _ptr(D), _ptr(mass), _ptr(alpha_T), _ptr(mbar), _ptr(grav), _ptr(dz), _ptr(tr), _ptr(d))
+        assert rc == 0
+        return (tr, d) if want_d else tr

@@ -572,3 +572,60 @@ int orc_photo_rates(int n_photo, int n_bins, int n_abs, const int *abs_species, 
   free(acc);
   return 0;
 }
+
+/* ---------------------------------------------------------------- f3: vertical (molecular-diffusion) transport terms
+ * PAPER.md:73-83.  Eq. 4:
+ *   d_{k+-1/2} = D_{k+-1/2} / (2 dz^2) * [ (mbar - m_y) g dz / (k_B T_{k+-1/2}) - alpha_T / T_{k+-1/2} * (T_{k+-1} - T_k) ]
+ * "k +- 1/2 refers to the arithmetic mean of k and k +- 1".  Eq. 3, the part that is
+ * not P - L:
+ *   tr_{y,k} = - d_{k+1/2} (N_{k+1/2} / N_{k+1}) n_{y,k+1}
+ *              - [ d_{k+1/2} (N_{k+1/2} / N_k) - d_{k-1/2} (N_{k-1/2} / N_k) ] n_{y,k}
+ *              + d_{k-1/2} (N_{k-1/2} / N_k) n_{y,k-1}
+ * with N = n_gas.  The printed equation is garbled in two places (reading V1): it carries an
+ * index "n_gas,j" where only k makes sense and a stray "/2" under the first term; both are dropped, everything
+ * else is taken literally.  Eddy diffusion does not appear ("the movement of the air parcel itself accounts for
+ * this process").  Zero-flux boundaries: the half-level coefficients outside the
+ * atmosphere are 0, so the terms that would reach below layer 0 or above the top layer vanish (reading V2).
+ * mbar and g are per atmosphere, dz is the uniform layer spacing of an atmosphere (Eq. 4 has one dz), D is
+ * given per (species, layer) (the paper computes it from Chapman-Enskog or binary-mixture theory, PAPER.md:67;
+ * here it is an input, reading V3), alpha_T per species.
+ * Layout: column = atmosphere * n_layers + layer, layer 0 at the bottom; tr [n_species][ld].
+ * d_out (optional) [n_species][ld]: d_{k+1/2} of every layer (0 at the top layer).
+ * Pins (tests/test_oracle_transport.py): Eq. 4 evaluated by hand; d = 0 for m_y = mbar in an isothermal column;
+ * the uniform-N reduction -d+ n_{k+1} - (d+ - d-) n_k + d- n_{k-1}; linearity in n; a three-layer column
+ * expanded by hand; zero-flux rows; independence of atmospheres. */
+int orc_transport(int n_species, long n_atm, long n_layers, long ld, const double *n, const double *T,
+                  const double *n_gas, const double *D, const double *mass, const double *alpha_T,
+                  const double *mbar, const double *grav, const double *dz, double *tr, double *d_out) {
+  for (long a = 0; a < n_atm; ++a) {
+    real_t h = (real_t)dz[a];
+    for (int y = 0; y < n_species; ++y) {
+      const double *ny = n + (long)y * ld, *Dy = D + (long)y * ld;
+      for (long k = 0; k < n_layers; ++k) {
+        long c = a * n_layers + k;
+        real_t dp = 0, dm = 0, Np = 0, Nm = 0; /* d_{k+1/2}, d_{k-1/2}, N_{k+1/2}, N_{k-1/2} */
+        if (k + 1 < n_layers) {
+          real_t Th = ((real_t)T[c] + (real_t)T[c + 1]) / 2, Dh = ((real_t)Dy[c] + (real_t)Dy[c + 1]) / 2;
+          Np = ((real_t)n_gas[c] + (real_t)n_gas[c + 1]) / 2;
+          dp = Dh / (2 * h * h) *
+               (((real_t)mbar[a] - (real_t)mass[y]) * (real_t)grav[a] * h / (K_BOLTZ * Th) -
+                (real_t)alpha_T[y] / Th * ((real_t)T[c + 1] - (real_t)T[c]));
+        }
+        if (k > 0) {
+          real_t Th = ((real_t)T[c] + (real_t)T[c - 1]) / 2, Dh = ((real_t)Dy[c] + (real_t)Dy[c - 1]) / 2;
+          Nm = ((real_t)n_gas[c] + (real_t)n_gas[c - 1]) / 2;
+          dm = Dh / (2 * h * h) *
+               (((real_t)mbar[a] - (real_t)mass[y]) * (real_t)grav[a] * h / (K_BOLTZ * Th) -
+                (real_t)alpha_T[y] / Th * ((real_t)T[c - 1] - (real_t)T[c]));
+        }
+        real_t Nk = (real_t)n_gas[c], t = 0;
+        if (k + 1 < n_layers) t -= dp * (Np / (real_t)n_gas[c + 1]) * (real_t)ny[c + 1];
+        t -= (dp * (Np / Nk) - dm * (Nm / Nk)) * (real_t)ny[c];
+        if (k > 0) t += dm * (Nm / Nk) * (real_t)ny[c - 1];
+        tr[(long)y * ld + c] = (double)t;
+        if (d_out) d_out[(long)y * ld + c] = (double)dp;
+      }
+    }
+  }
+  return 0;
+}
