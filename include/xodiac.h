@@ -150,7 +150,7 @@ enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD
        XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
        XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_JAC_TILED = 9, XOD_KERNEL_NEWTON_ASSEMBLE = 10,
        XOD_KERNEL_LU_FACTOR = 11, XOD_KERNEL_LU_SOLVE = 12, XOD_KERNEL_PHOTO_GEMM = 13, XOD_KERNEL_PHOTO_FLUX = 14,
-       XOD_KERNEL_COUNT = 15 };
+       XOD_KERNEL_TRANSPORT = 15, XOD_KERNEL_COUNT = 16 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);
@@ -260,6 +260,25 @@ size_t xod_photo_workspace_bytes(const xod_photo *photo, int64_t ncol);
 xod_status xod_photo_rates(const xod_photo *photo, int64_t n_atm, int64_t n_layers, int64_t ld, const double *n,
                            const double *dz, const double *j0, const double *j_diff, const double *mu,
                            const double *t_f, double *J, void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- f3: the molecular-diffusion transport terms of the continuity equation
+ * (PAPER.md:73-83).  Eq. 4, half levels k +- 1/2 being arithmetic means of k and k +- 1:
+ *   d_{k+-1/2} = D_{k+-1/2} / (2 dz^2) [ (mbar - m_y) g dz / (k_B T_{k+-1/2}) - alpha_T / T_{k+-1/2} (T_{k+-1} - T_k) ]
+ * and the part of Eq. 3 that is not P - L, with N = n_gas:
+ *   tr_{y,k} = - d_{k+1/2} (N_{k+1/2}/N_{k+1}) n_{y,k+1} - [ d_{k+1/2} (N_{k+1/2}/N_k) - d_{k-1/2} (N_{k-1/2}/N_k) ] n_{y,k}
+ *              + d_{k-1/2} (N_{k-1/2}/N_k) n_{y,k-1}
+ * so that dn/dt of Eq. 1 = (xod_source's dn/dt) + tr.  Two extraction garbles of the printed Eq. 3 (an index
+ * "n_gas,j" and a stray "/2") are dropped (reading V1); zero-flux boundaries: no term reaches
+ * across the bottom or top layer of an atmosphere (V2); eddy diffusion does not appear.
+ * Column = atmosphere * n_layers + layer, layer 0 at the bottom.  n, D [n_species][ld] (D: molecular diffusion
+ * coefficient of each species in each layer, cm^2 s^-1, an input: reading V3), T, n_gas [ld], mass, alpha_T
+ * [n_species] (g; thermal diffusion factor), mbar, grav, dz [n_atm] (mean molecular mass in g, gravity in cm s^-2,
+ * uniform layer spacing in cm), tr [n_species][ld] out: device memory owned by the caller; columns >= n_atm *
+ * n_layers are not touched.  Errors: XOD_ERR_INVALID_ARG, XOD_ERR_CUDA. */
+xod_status xod_transport(const xod_network *net, int64_t n_atm, int64_t n_layers, int64_t ld, const double *n,
+                         const double *T, const double *n_gas, const double *D, const double *mass,
+                         const double *alpha_T, const double *mbar, const double *grav, const double *dz, double *tr,
+                         void *stream);
 
 /* ---- end-to-end convenience: the fused call on HOST buffers (pinned for overlap; pageable works
  * but serialises).  Columns are processed in chunks of one round of tiles per SM through three

@@ -11,6 +11,7 @@
 #include "jac_tiled.cuh"
 #include "newton.cuh"
 #include "photo.cuh"
+#include "transport.cuh"
 #include "rates2.cuh"
 #include "kernels.cuh"
 
@@ -998,6 +999,36 @@ xod_status xod_photo_rates(const xod_photo *ph, int64_t n_atm, int64_t n_layers,
     k_photo_gemm<true><<<grid, 256, 0, s>>>(g);
     XOD_CUDA(cudaGetLastError());
   }
+  return XOD_OK;
+}
+
+// ---------------------------------------------------------------------------- f3: transport terms
+
+xod_status xod_transport(const xod_network *net, int64_t n_atm, int64_t n_layers, int64_t ld, const double *n,
+                         const double *T, const double *n_gas, const double *D, const double *mass,
+                         const double *alpha_T, const double *mbar, const double *grav, const double *dz, double *tr,
+                         void *stream) {
+  if (n_atm < 0 || n_layers < 0) return fail(XOD_ERR_INVALID_ARG, "n_atm or n_layers < 0");
+  const int64_t ncol = n_atm * n_layers;
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (ncol == 0) return XOD_OK;
+  if (!n || !T || !n_gas || !D || !mass || !alpha_T || !mbar || !grav || !dz || !tr)
+    return fail(XOD_ERR_INVALID_ARG, "n, T, n_gas, D, mass, alpha_T, mbar, grav, dz or tr is NULL");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  TransportArgs a{};
+  a.ncol = ncol, a.n_layers = n_layers, a.ld = ld, a.ns = net->h.ns;
+  a.n = n, a.T = T, a.n_gas = n_gas, a.D = D, a.mass = mass, a.alpha_T = alpha_T, a.mbar = mbar, a.grav = grav, a.dz = dz, a.tr = tr;
+  const int64_t gx = (ncol + 127) / 128;
+  int spb = net->h.ns;   // enough CTAs to fill the chip even for one atmosphere: split the species over blockIdx.y
+  while (spb > 4 && gx * ((net->h.ns + spb - 1) / spb) < (int64_t)net->sm_count * 8) spb = (spb + 1) / 2;
+  a.spb = spb;
+  dim3 grid((unsigned)gx, (unsigned)((net->h.ns + spb - 1) / spb));
+  {
+    Timed tm(net, KID_TRANSPORT, s);
+    k_transport<<<grid, 128, 0, s>>>(a);
+  }
+  XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
 

@@ -214,7 +214,7 @@ size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_TRANSPORT, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused

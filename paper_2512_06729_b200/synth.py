@@ -771,3 +771,34 @@ def make_irradiation(seed, net, atm, photo, with_diffuse=True):
         for a in range(n_atm):
             j_diff[:, a * L:(a + 1) * L] = j0[a][:, None] * rng.uniform(0.0, 0.05, size=(photo.n_bins, L))
     return dz, j0, j_diff, mu, t_f
+
+
+# --------------------------------------------------------------------------- f3: transport inputs
+
+def make_transport(seed, net, atm):
+    """Seeded inputs of the molecular-diffusion terms for an atmosphere of make_atmosphere: species
+    masses from the composition (standard atomic masses of the element labels; 1 u for unknown labels and for the
+    charge column), a mean molecular mass of 2.2-2.4 u and a gravity of 500-2500 cm s^-2 per atmosphere, the uniform
+    layer spacing that the log-pressure grid implies for the column's mean temperature, thermal diffusion factors
+    uniform -0.4..0.3 (alpha_T = -0.38 for light species is the usual choice), the gas density n_gas = P / (k_B T),
+    and binary-mixture-like diffusion coefficients D = b T^0.75 / n_gas with b log-uniform 1e17..1e18 per species
+    (the paper takes its parameters from several sources; none is reproduced here)."""
+    rng = np.random.default_rng(seed)
+    amu = {"H": 1.008, "He": 4.0026, "C": 12.011, "N": 14.007, "O": 15.999, "P": 30.974, "S": 32.06, "Na": 22.990,
+           "K": 39.098, "Fe": 55.845}
+    w = np.array([amu.get(e, 0.0) for e in net.element_names])
+    mass = np.maximum(np.abs(net.composition) @ w, 1.0) * 1.66053907e-24
+    n_atm, L = atm.meta["n_atm"], atm.meta["n_layers"]
+    mbar = rng.uniform(2.2, 2.4, size=n_atm) * 1.66053907e-24
+    grav = rng.uniform(500.0, 2500.0, size=n_atm)
+    dz = np.zeros(n_atm)
+    dlnp = np.log(1.0e11) / max(L - 1, 1)
+    for a in range(n_atm):
+        dz[a] = dlnp * K_B * atm.T[a * L:(a + 1) * L].mean() / (mbar[a] * grav[a])
+    alpha_T = rng.uniform(-0.4, 0.3, size=net.n_species)
+    n_gas = np.ones(atm.ld)
+    n_gas[:atm.ncol] = atm.P[:atm.ncol] / (K_B * atm.T[:atm.ncol])
+    D = np.ones((net.n_species, atm.ld))
+    b = _loguniform(rng, 1e17, 1e18, size=net.n_species)
+    D[:, :atm.ncol] = b[:, None] * atm.T[None, :atm.ncol] ** 0.75 / n_gas[None, :atm.ncol]
+    return dict(mass=mass, alpha_T=alpha_T, mbar=mbar, grav=grav, dz=dz, n_gas=n_gas, D=D)

@@ -20,6 +20,7 @@ void emu_syncthreads() { g_barrier->arrive_and_wait(); }
 #include "../../paper_2512_06729_b200/csrc/jac_tiled.cuh"
 #include "../../paper_2512_06729_b200/csrc/newton.cuh"
 #include "../../paper_2512_06729_b200/csrc/photo.cuh"
+#include "../../paper_2512_06729_b200/csrc/transport.cuh"
 #include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
@@ -284,6 +285,19 @@ int emu_photo_rates(int ns, int n_photo, int n_bins, int n_abs, const int32_t *a
     run_grid((unsigned)((ncol + kGemmBN - 1) / kGemmBN), (unsigned)((n_photo + kGemmBM - 1) / kGemmBM), 256, true,
              [&] { k_photo_gemm<true>(g); });
   }
+  return 0;
+}
+
+// f3: transport terms by k_transport (thread = column, species blocks over blockIdx.y)
+int emu_transport(int ns, int64_t n_atm, int64_t n_layers, int64_t ld, const double *n, const double *T, const double *n_gas,
+                  const double *D, const double *mass, const double *alpha_T, const double *mbar, const double *grav,
+                  const double *dz, double *tr, int spb) {
+  TransportArgs a{};
+  a.ncol = n_atm * n_layers, a.n_layers = n_layers, a.ld = ld, a.ns = ns;
+  a.n = n, a.T = T, a.n_gas = n_gas, a.D = D, a.mass = mass, a.alpha_T = alpha_T, a.mbar = mbar, a.grav = grav, a.dz = dz, a.tr = tr;
+  a.spb = spb;
+  if (a.ncol <= 0) return 1;
+  run_grid((unsigned)((a.ncol + 127) / 128), (unsigned)((ns + spb - 1) / spb), 128, false, [&] { k_transport(a); });
   return 0;
 }
 
