@@ -230,3 +230,18 @@ class Oracle:
                                     _ptr(D), _ptr(mass), _ptr(alpha_T), _ptr(mbar), _ptr(grav), _ptr(dz), _ptr(tr), _ptr(d))
         assert rc == 0
         return (tr, d) if want_d else tr
+
+    # ---- f4: reaction pathway analyser
+    def pathway(self, net, kf, kr, n, source, ncol=None):
+        """dist [n_species][ld] (sum of 1/rate along the fastest route from `source`), pred, via (int32)."""
+        kf, kr, n = _f64(kf), _f64(kr), _f64(n)
+        ld = n.shape[1]
+        ncol = ld if ncol is None else ncol
+        ns, _ = self._dims(net)
+        s, keep = self._net(net)
+        dist = np.full((ns, ld), np.nan)
+        pred, via = np.full((ns, ld), -2, dtype=np.int32), np.full((ns, ld), -2, dtype=np.int32)
+        rc = self.lib.orc_pathway(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(kf), _ptr(kr), _ptr(n), C.c_int(source),
+                                  _ptr(dist), _ptr(pred), _ptr(via))
+        assert rc == 0
+        return dist, pred, via

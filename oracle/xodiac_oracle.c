@@ -629,3 +629,76 @@ int orc_transport(int n_species, long n_atm, long n_layers, long ld, const doubl
   }
   return 0;
 }
+
+/* ---------------------------------------------------------------- f4: reaction pathway analyser
+ * "a reaction pathway analyzer designed to identify the most efficient conversion routes between any
+ * two species ... built upon Dijkstra's classic algorithm (Dijkstra 1959), which identifies the kinetically fastest
+ * reaction pathway by minimizing the cumulative sum of inverse reaction rates"; "The rate-limiting
+ * step, defined as the slowest reaction in each pathway".
+ * Graph of one column (reading W1; the paper does not spell it out): nodes are species; every listed
+ * reaction contributes, for its forward direction with rate q_f = k_f prod n_reactant and (if reversible) its reverse
+ * direction with q_r = k_r prod n_product (O4), a directed edge from each distinct species it consumes to each
+ * distinct species it forms in that direction (u != v), of weight 1 / q.  A direction whose rate is not a positive
+ * finite number offers no edge.  Parallel edges: the lighter one counts.
+ * The oracle is Dijkstra's algorithm as in any textbook, one column and one source at a time, with a linear scan for
+ * the closest unsettled node; distances are accumulated in real_t from the source outwards.
+ * Outputs [n_species][ld]: dist (0 at the source, +inf if unreachable), pred (previous species on the path, -1 for
+ * the source and for unreachable species), via (user reaction index of the last edge, bit 30 set for the reverse
+ * direction; -1 likewise).  Ties between equally short paths are broken by the scan order (lowest species index
+ * settled first, first edge found kept); only dist is unique.
+ * Pins (tests/test_oracle_pathway.py): a hand graph where the two-step route beats the direct one exactly when
+ * 1/q1 + 1/q2 < 1/q3; the min-plus closure (Floyd-Warshall in numpy) of the same edge weights from every source;
+ * the optimality conditions dist[v] <= dist[u] + w on every edge with equality on the tree; dist scales as 1/c when
+ * all rates are multiplied by c; unreachable species; the rate-limiting step of a path. */
+int orc_pathway(const orc_network *net, long ncol, long ld, const double *kf, const double *kr, const double *n,
+                int source, double *dist_out, int *pred_out, int *via_out) {
+  int ns = net->n_species, nr = net->n_reactions;
+  real_t *dist = (real_t *)malloc(sizeof(real_t) * (size_t)ns);
+  real_t *w = (real_t *)malloc(sizeof(real_t) * (size_t)nr * 2);
+  unsigned char *done = (unsigned char *)malloc((size_t)ns);
+  int *pred = (int *)malloc(sizeof(int) * (size_t)ns * 2), *via = pred + ns;
+  if (!dist || !w || !done || !pred) return -1;
+  if (source < 0 || source >= ns) return -2;
+  for (long c = 0; c < ncol; ++c) {
+    for (int r = 0; r < nr; ++r) { /* edge weights of this column: 1 / rate of progress, per direction */
+      real_t qf = rate_of(net->reactants + 3 * r, kf[(long)r * ld + c], n, ld, c);
+      real_t qr = net->reversible[r] ? rate_of(net->products + 3 * r, kr[(long)r * ld + c], n, ld, c) : 0;
+      w[2 * r] = (qf > 0 && qf == qf && 1 / qf > 0) ? 1 / qf : (real_t)INFINITY;
+      w[2 * r + 1] = (qr > 0 && qr == qr && 1 / qr > 0) ? 1 / qr : (real_t)INFINITY;
+    }
+    for (int i = 0; i < ns; ++i) dist[i] = (real_t)INFINITY, done[i] = 0, pred[i] = via[i] = -1;
+    dist[source] = 0;
+    for (;;) {
+      int u = -1;
+      for (int i = 0; i < ns; ++i)
+        if (!done[i] && dist[i] < (real_t)INFINITY && (u < 0 || dist[i] < dist[u])) u = i;
+      if (u < 0) break;
+      done[u] = 1;
+      for (int r = 0; r < nr; ++r)
+        for (int d = 0; d < 2; ++d) {
+          if (!(w[2 * r + d] < (real_t)INFINITY)) continue;
+          const int *from = d ? net->products + 3 * r : net->reactants + 3 * r;
+          const int *to = d ? net->reactants + 3 * r : net->products + 3 * r;
+          int consumes = 0;
+          for (int a = 0; a < 3; ++a) consumes |= from[a] == u;
+          if (!consumes) continue;
+          for (int b = 0; b < 3; ++b) {
+            int v = to[b];
+            if (v < 0 || v == u || done[v]) continue;
+            real_t cand = dist[u] + w[2 * r + d];
+            if (cand < dist[v]) dist[v] = cand, pred[v] = u, via[v] = r | (d ? (1 << 30) : 0);
+          }
+        }
+    }
+    for (int i = 0; i < ns; ++i) {
+      dist_out[(long)i * ld + c] = (double)dist[i];
+      if (pred_out) pred_out[(long)i * ld + c] = pred[i];
+      if (via_out) via_out[(long)i * ld + c] = via[i];
+    }
+  }
+  free(dist);
+  free(w);
+  free(done);
+  free(pred);
+  return 0;
+}
