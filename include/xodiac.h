@@ -150,7 +150,7 @@ enum { XOD_KERNEL_THERMO = 0, XOD_KERNEL_PROLOGUE = 1, XOD_KERNEL_RATES = 2, XOD
        XOD_KERNEL_SOURCE = 4, XOD_KERNEL_JACOBIAN = 5, XOD_KERNEL_FUSED = 6, XOD_KERNEL_FUSED_COMBINE = 7,
        XOD_KERNEL_RATE_COEFFS = 8, XOD_KERNEL_JAC_TILED = 9, XOD_KERNEL_NEWTON_ASSEMBLE = 10,
        XOD_KERNEL_LU_FACTOR = 11, XOD_KERNEL_LU_SOLVE = 12, XOD_KERNEL_PHOTO_GEMM = 13, XOD_KERNEL_PHOTO_FLUX = 14,
-       XOD_KERNEL_TRANSPORT = 15, XOD_KERNEL_COUNT = 16 };
+       XOD_KERNEL_TRANSPORT = 15, XOD_KERNEL_PATH_WEIGHTS = 16, XOD_KERNEL_PATHWAY = 17, XOD_KERNEL_COUNT = 18 };
 xod_status xod_network_timing_read(xod_network *net, double *ms, int64_t *launches);
 /* kernels launched by this library in this process so far (all networks, all threads) */
 int64_t xod_launch_count(void);
@@ -279,6 +279,28 @@ xod_status xod_transport(const xod_network *net, int64_t n_atm, int64_t n_layers
                          const double *T, const double *n_gas, const double *D, const double *mass,
                          const double *alpha_T, const double *mbar, const double *grav, const double *dz, double *tr,
                          void *stream);
+
+/* ---- f4: the reaction pathway analyser.  "identifies the kinetically fastest reaction
+ * pathway by minimizing the cumulative sum of inverse reaction rates" (after Dijkstra 1959); "the
+ * rate-limiting step, defined as the slowest reaction in each pathway".
+ * Graph of a column (reading W1): nodes = species; every reaction direction with a positive finite rate of
+ * progress q (q_f = k_f prod n_reactant, q_r = k_r prod n_product, reversible reactions only) gives a directed edge of
+ * weight 1/q from each distinct species it consumes to each distinct species it forms.  For every column the call
+ * returns, for all species v, dist[v][col] = the smallest sum of weights over routes source -> v (0 for the source,
+ * +inf if unreachable), pred[v][col] = the species before v on such a route and via[v][col] = the USER index of its
+ * last reaction, bit 30 set for the reverse direction (both -1 for the source and for unreachable species).  Walking
+ * pred back from a target lists the route; its largest 1/q step is the rate-limiting one.  dist is unique; when
+ * several routes are equally short, pred/via name one of them (fixed, deterministic choice).
+ * kf, kr [n_reactions][ld], n, dist [n_species][ld] fp64, pred, via [n_species][ld] int32: device memory owned by the
+ * caller; workspace >= xod_pathway_workspace_bytes (the edge weights, [2 n_reactions][columns]).
+ * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, source out of range, tables unavailable: n_species or 2 n_reactions
+ * >= 65535, or the tiles exceed shared memory), XOD_ERR_WORKSPACE, XOD_ERR_CUDA.
+ * The equilibrium-chemistry start (NEXOCHEM / FASTCHEM) named beside it in SURVEY f4 is not built:
+ * the paper gives no algorithm for it. */
+size_t xod_pathway_workspace_bytes(const xod_network *net, int64_t ncol);
+xod_status xod_pathway(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                       const double *n, int32_t source, double *dist, int32_t *pred, int32_t *via, void *workspace,
+                       size_t workspace_bytes, void *stream);
 
 /* ---- end-to-end convenience: the fused call on HOST buffers (pinned for overlap; pageable works
  * but serialises).  Columns are processed in chunks of one round of tiles per SM through three

@@ -661,10 +661,14 @@ int orc_pathway(const orc_network *net, long ncol, long ld, const double *kf, co
   if (source < 0 || source >= ns) return -2;
   for (long c = 0; c < ncol; ++c) {
     for (int r = 0; r < nr; ++r) { /* edge weights of this column: 1 / rate of progress, per direction */
-      real_t qf = rate_of(net->reactants + 3 * r, kf[(long)r * ld + c], n, ld, c);
-      real_t qr = net->reversible[r] ? rate_of(net->products + 3 * r, kr[(long)r * ld + c], n, ld, c) : 0;
-      w[2 * r] = (qf > 0 && qf == qf && 1 / qf > 0) ? 1 / qf : (real_t)INFINITY;
-      w[2 * r + 1] = (qr > 0 && qr == qr && 1 / qr > 0) ? 1 / qr : (real_t)INFINITY;
+      /* the rates are rounded to double first: whether a direction "has a positive finite rate" is decided in the
+       * path's arithmetic type (fp64), like every other quantity the library hands out (q beyond the double range is
+       * +inf and offers no edge, exactly as a caller computing 1/q from xod's own outputs would see it) */
+      double qf = (double)rate_of(net->reactants + 3 * r, kf[(long)r * ld + c], n, ld, c);
+      double qr = net->reversible[r] ? (double)rate_of(net->products + 3 * r, kr[(long)r * ld + c], n, ld, c) : 0;
+      double wf = 1 / qf, wr = 1 / qr;
+      w[2 * r] = (qf > 0 && wf > 0 && wf < INFINITY) ? (real_t)1 / (real_t)qf : (real_t)INFINITY;
+      w[2 * r + 1] = (qr > 0 && wr > 0 && wr < INFINITY) ? (real_t)1 / (real_t)qr : (real_t)INFINITY;
     }
     for (int i = 0; i < ns; ++i) dist[i] = (real_t)INFINITY, done[i] = 0, pred[i] = via[i] = -1;
     dist[source] = 0;

@@ -17,7 +17,7 @@ XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK, XOD_FLAG_BUILD_LU = 1, 2
 XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL, XOD_TUNE_JAC_TILED = 0, 1, 2, 3, 4
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve", "photo_gemm", "photo_flux", "transport"]
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve", "photo_gemm", "photo_flux", "transport", "path_weights", "pathway"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -29,7 +29,8 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_source_fused_host", "xod_probe_fp64_peak", "xod_network_timing_read", "xod_launch_count", "xod_network_fused_info", "xod_network_selfcheck", "xod_network_fused_params",
            "xod_check_status", "xod_build_has_checks", "xod_network_jac_info", "xod_network_lu_info", "xod_network_lu_pattern",
            "xod_newton_workspace_bytes", "xod_newton_step", "xod_photo_create", "xod_photo_destroy",
-           "xod_photo_workspace_bytes", "xod_photo_rates", "xod_transport"]
+           "xod_photo_workspace_bytes", "xod_photo_rates", "xod_transport",
+           "xod_pathway_workspace_bytes", "xod_pathway"]
 
 
 class XodError(RuntimeError):
@@ -57,7 +58,7 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         L.xod_last_error.restype = C.c_char_p
         for name in ("xod_rate_coeffs_workspace_bytes", "xod_source_workspace_bytes",
-                     "xod_source_fused_workspace_bytes", "xod_newton_workspace_bytes"):
+                     "xod_source_fused_workspace_bytes", "xod_newton_workspace_bytes", "xod_pathway_workspace_bytes"):
             getattr(L, name).restype = C.c_size_t
             getattr(L, name).argtypes = [C.c_void_p, C.c_int64]
         L.xod_photo_workspace_bytes.restype = C.c_size_t
@@ -257,6 +258,16 @@ class Network:
     def transport(self, n_atm, n_layers, ld, n, T, n_gas, D, mass, alpha_T, mbar, grav, dz, tr, stream=None):
         _check(lib().xod_transport(self._h, C.c_int64(n_atm), C.c_int64(n_layers), C.c_int64(ld), _dp(n), _dp(T), _dp(n_gas),
                                    _dp(D), _dp(mass), _dp(alpha_T), _dp(mbar), _dp(grav), _dp(dz), _dp(tr), _stream(stream)))
+
+    # ---- f4: pathway analyser (dist fp64, pred / via int32 tensors)
+    def pathway_workspace_bytes(self, ncol):
+        return lib().xod_pathway_workspace_bytes(self._h, ncol)
+
+    def pathway(self, ncol, ld, kf, kr, n, source, dist, pred, via, workspace, stream=None):
+        assert pred.is_cuda and via.is_cuda and pred.element_size() == 4 and via.element_size() == 4
+        _check(lib().xod_pathway(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(kf), _dp(kr), _dp(n), C.c_int32(source), _dp(dist),
+                                 C.c_void_p(pred.data_ptr()), C.c_void_p(via.data_ptr()), _dp(workspace),
+                                 C.c_size_t(0 if workspace is None else workspace.numel() * 8), _stream(stream)))
 
     # ---- end to end on HOST buffers (numpy arrays or pinned torch CPU tensors)
     def source_fused_host(self, ncol, ld, T, P, J, n, dndt):

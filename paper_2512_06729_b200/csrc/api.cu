@@ -12,6 +12,7 @@
 #include "newton.cuh"
 #include "photo.cuh"
 #include "transport.cuh"
+#include "pathway.cuh"
 #include "rates2.cuh"
 #include "kernels.cuh"
 
@@ -187,6 +188,8 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (net->h.jt.enabled && jac_tiled_smem_bytes(net->h.ns, net->h.jt.acc_rows, chunk, net->h.jt.meta_cap) <= kFusedSmemMax) break;
       net->h.jt.enabled = false;
     }
+    pack_path(desc, net->h);
+    if (net->h.path.enabled && path_smem_bytes(net->h.ns) > kFusedSmemMax) net->h.path.enabled = false;
     if (desc->flags & XOD_FLAG_BUILD_LU) {
       pack_lu(net->h);
       if (!net->h.lu.enabled) {
@@ -264,6 +267,18 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (st == XOD_OK) {
         cudaError_t ce = cudaFuncSetAttribute(k_jac_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
         if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_jac_tiled)");
+      }
+    }
+    if (h.path.enabled) {
+      PathHost &ph = h.path;
+      PathDev &pd = net->pd;
+      pd.enabled = 1, pd.n_steps = ph.n_steps, pd.n_edges = ph.n_edges;
+      if (st == XOD_OK) st = upload(net, ph.in_u, &pd.in_u);
+      if (st == XOD_OK) st = upload(net, ph.in_rd, &pd.in_rd);
+      if (st == XOD_OK) st = upload(net, ph.sched, &pd.sched);
+      if (st == XOD_OK) {
+        cudaError_t ce = cudaFuncSetAttribute(k_pathway, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
+        if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_pathway)");
       }
     }
     if (h.lu.enabled) {
@@ -1029,6 +1044,50 @@ xod_status xod_transport(const xod_network *net, int64_t n_atm, int64_t n_layers
     k_transport<<<grid, 128, 0, s>>>(a);
   }
   XOD_CUDA(cudaGetLastError());
+  return XOD_OK;
+}
+
+// ---------------------------------------------------------------------------- f4: pathway analyser
+
+size_t xod_pathway_workspace_bytes(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0 || !net->h.path.enabled) return 0;
+  return (size_t)2 * net->h.nr * (size_t)round_up(std::max<int64_t>(ncol, 1), 32) * sizeof(double) + 256;
+}
+
+xod_status xod_pathway(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,
+                       const double *n, int32_t source, double *dist, int32_t *pred, int32_t *via, void *workspace,
+                       size_t workspace_bytes, void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (!net->h.path.enabled) return fail(XOD_ERR_INVALID_ARG, "the pathway tables do not fit (too many species or reactions)");
+  if (source < 0 || source >= net->h.ns) return fail(XOD_ERR_INVALID_ARG, "source species out of range");
+  if (ncol == 0) return XOD_OK;
+  if (!n || !dist || !pred || !via) return fail(XOD_ERR_INVALID_ARG, "n, dist, pred or via is NULL");
+  if (net->h.nr > 0 && (!kf || !kr)) return fail(XOD_ERR_INVALID_ARG, "kf or kr is NULL");
+  if (!workspace || workspace_bytes < xod_pathway_workspace_bytes(net, ncol))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_pathway_workspace_bytes");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  PathArgs a{};
+  a.ncol = ncol, a.ld = ld, a.ldw = round_up(ncol, 32);
+  a.kf = kf, a.kr = kr, a.n = n;
+  a.w = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
+  a.dist = dist, a.pred = pred, a.via = via, a.source = source, a.ns = net->h.ns, a.nr = net->h.nr;
+  a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
+  if (net->h.nr > 0) {
+    const int64_t gx = (ncol + 127) / 128;
+    int rslice = net->h.nr;
+    while (rslice > 16 && gx * ((net->h.nr + rslice - 1) / rslice) < (int64_t)net->sm_count * 8) rslice = (rslice + 1) / 2;
+    dim3 grid((unsigned)gx, (unsigned)((net->h.nr + rslice - 1) / rslice));
+    Timed tm(net, KID_PATH_WEIGHTS, s);
+    k_path_weights<<<grid, 128, 0, s>>>(net->d, a, rslice);
+    XOD_CUDA(cudaGetLastError());
+  }
+  {
+    const unsigned grid = (unsigned)std::min<int64_t>(a.ntiles, net->sm_count);
+    Timed tm(net, KID_PATHWAY, s);
+    k_pathway<<<grid, kFWarps * 32, path_smem_bytes(net->h.ns), s>>>(net->pd, a);
+    XOD_CUDA(cudaGetLastError());
+  }
   return XOD_OK;
 }
 

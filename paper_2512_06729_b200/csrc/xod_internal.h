@@ -166,6 +166,26 @@ struct LuDev {
   const uint16_t *tgt;
 };
 
+// ---- tables of the pathway analyser (f4: xod_pathway; pack_path.cpp, pathway.cuh) ----------------
+// Incoming-edge lists per destination species and a step schedule for a CTA of kFWarps warps: in every step a
+// warp relaxes one part of one node's incoming edges (its four lane groups take every fourth edge); the parts of a
+// node sit on consecutive warps of the same step and are combined in a fixed order by the first of them.
+struct PathTask { int32_t node, begin, end, first_warp_parts; };   // first_warp_parts: first warp of the node | parts << 16; node < 0: idle
+struct PathHost {
+  bool enabled = false;
+  int32_t n_steps = 0;
+  int64_t n_edges = 0;
+  std::vector<int64_t> in_ptr;          // [ns + 1]
+  std::vector<uint16_t> in_u, in_rd;    // [n_edges]: source species; 2 * user reaction + direction
+  std::vector<PathTask> sched;          // [n_steps][kFWarps]
+};
+struct PathDev {
+  int32_t enabled, n_steps;
+  int64_t n_edges;
+  const uint16_t *in_u, *in_rd;
+  const PathTask *sched;
+};
+
 struct HostTables {
   int32_t ns = 0, ne = 0, nr = 0, n_photo = 0;
   int32_t uni_begin = 0, bi_begin = 0, fo_begin = 0, ph_begin = 0;
@@ -187,6 +207,7 @@ struct HostTables {
   FusedHost f;
   JacTiledHost jt;
   LuHost lu;
+  PathHost path;
 };
 
 // one row task of a chunk schedule: an accumulator row and its entries (q row | nu bits)
@@ -207,6 +228,9 @@ void pack_jac_tiled(HostTables &h, int chunk, int acc_budget);
 bool check_jac_tiled(const HostTables &h, std::string &err);
 // pack_lu.cpp: minimum-degree ordering, filled pattern and update schedule of the implicit step
 void pack_lu(HostTables &h);
+// pack_path.cpp: incoming-edge lists and step schedule of the pathway analyser
+void pack_path(const xod_network_desc *d, HostTables &h);
+size_t path_smem_bytes(int ns);
 size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 
 }  // namespace xod
@@ -214,7 +238,7 @@ size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_TRANSPORT, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_TRANSPORT, KID_PATH_WEIGHTS, KID_PATHWAY, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused
@@ -242,6 +266,7 @@ struct xod_network {
   xod::FusedDev fd{};
   xod::JacTiledDev jd{};
   xod::LuDev ld{};
+  xod::PathDev pd{};
   int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
   int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
   int64_t use_jac_tiled = 1;  // XOD_TUNE_JAC_TILED: 0 = the one-warp-per-entry gather kernel

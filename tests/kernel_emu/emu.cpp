@@ -3,6 +3,7 @@
 // the host packer builds the tables exactly as xod_network_create does, then k_fused /
 // k_fused_combine / k_rate_coeffs are executed with one std::thread per CUDA thread of a block
 // (blocks one after another) and a std::barrier as __syncthreads.
+#include <atomic>
 #include <barrier>
 #include <memory>
 #include <thread>
@@ -14,6 +15,16 @@ thread_local emu_dim threadIdx, blockIdx;
 emu_dim gridDim, blockDim;
 static std::unique_ptr<std::barrier<>> g_barrier;
 void emu_syncthreads() { g_barrier->arrive_and_wait(); }
+static std::atomic<int> g_or{0};
+int emu_syncthreads_or(int predicate) {   // barrier with an OR reduction over the block
+  if (predicate) g_or.fetch_or(1);
+  g_barrier->arrive_and_wait();
+  const int r = g_or.load();
+  g_barrier->arrive_and_wait();
+  if (threadIdx.x == 0) g_or.store(0);
+  g_barrier->arrive_and_wait();
+  return r;
+}
 
 #include "../../paper_2512_06729_b200/csrc/fused.cuh"
 #include "../../paper_2512_06729_b200/csrc/rates2.cuh"
@@ -21,6 +32,7 @@ void emu_syncthreads() { g_barrier->arrive_and_wait(); }
 #include "../../paper_2512_06729_b200/csrc/newton.cuh"
 #include "../../paper_2512_06729_b200/csrc/photo.cuh"
 #include "../../paper_2512_06729_b200/csrc/transport.cuh"
+#include "../../paper_2512_06729_b200/csrc/pathway.cuh"
 #include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
@@ -298,6 +310,28 @@ int emu_transport(int ns, int64_t n_atm, int64_t n_layers, int64_t ld, const dou
   a.spb = spb;
   if (a.ncol <= 0) return 1;
   run_grid((unsigned)((a.ncol + 127) / 128), (unsigned)((ns + spb - 1) / spb), 128, false, [&] { k_transport(a); });
+  return 0;
+}
+
+// f4: pathway analyser: k_path_weights, then k_pathway on `grid` blocks
+int emu_pathway(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *kf, const double *kr, const double *n,
+                int source, double *dist, int32_t *pred, int32_t *via, int grid) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK || ncol <= 0) return 1;
+  pack_path(desc, h);
+  if (!h.path.enabled || path_smem_bytes(h.ns) > sizeof(smem_raw)) return 2;
+  const DevTables d = dev_tables(h);
+  PathDev pd{};
+  pd.enabled = 1, pd.n_steps = h.path.n_steps, pd.n_edges = h.path.n_edges;
+  pd.in_u = h.path.in_u.data(), pd.in_rd = h.path.in_rd.data(), pd.sched = h.path.sched.data();
+  PathArgs a{};
+  a.ncol = ncol, a.ld = ld, a.ldw = (ncol + 31) / 32 * 32, a.kf = kf, a.kr = kr, a.n = n;
+  std::vector<double> w((size_t)2 * h.nr * a.ldw, NAN);
+  a.w = w.data(), a.dist = dist, a.pred = pred, a.via = via, a.source = source, a.ns = h.ns, a.nr = h.nr;
+  a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
+  run_grid((unsigned)((ncol + 127) / 128), 3, 128, false, [&] { k_path_weights(d, a, (h.nr + 2) / 3); });
+  run_grid((unsigned)grid, 1, kFWarps * 32, true, [&] { k_pathway(pd, a); });
   return 0;
 }
 

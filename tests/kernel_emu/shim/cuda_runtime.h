@@ -29,7 +29,9 @@ inline int4 make_int4(int x, int y, int z, int w) { return int4{x, y, z, w}; }
 extern thread_local emu_dim threadIdx, blockIdx;
 extern emu_dim gridDim, blockDim;
 void emu_syncthreads();
+int emu_syncthreads_or(int predicate);
 #define __syncthreads() emu_syncthreads()
+#define __syncthreads_or(p) emu_syncthreads_or((p) ? 1 : 0)
 #define __syncwarp()
 
 template <class T> inline T __ldg(const T *p) { return *p; }
@@ -41,6 +43,7 @@ inline double __hiloint2double(int hi, int lo) {
 }
 inline int __double2hiint(double d) { uint64_t b; std::memcpy(&b, &d, 8); return (int)(b >> 32); }
 inline int __double2loint(double d) { uint64_t b; std::memcpy(&b, &d, 8); return (int)(uint32_t)b; }
+inline double __longlong_as_double(long long v) { double d; std::memcpy(&d, &v, 8); return d; }
 inline float __int_as_float(int i) { float f; std::memcpy(&f, &i, 4); return f; }
 inline size_t __cvta_generic_to_shared(const void *p) { return (size_t)p; }
 
