@@ -388,6 +388,37 @@ def next_row_timings(binding, net, dev, ws_for):
         h.close()
     except Exception as exc:
         out["f2_photo_rates"] = {"error": repr(exc)[:300]}
+    try:
+        atm = synth.make_atmosphere(2005, net, 64, 150)
+        t = synth.make_transport(61, net, atm)
+        h = binding.Network(net, device=torch.cuda.current_device())
+        tr = torch.empty((net.n_species, atm.ld), dtype=torch.float64, device="cuda")
+        args = [dev(x) for x in (atm.n, atm.T, t["n_gas"], t["D"], t["mass"], t["alpha_T"], t["mbar"], t["grav"], t["dz"])]
+        call = lambda: h.transport(64, 150, atm.ld, *args, tr)
+        call()
+        sync()
+        ms = event_time_ms(call, 5, sync)
+        out["f3_transport"] = {"ncol": atm.ncol, "ms": ms, "gbs": 24.0 * net.n_species * atm.ncol / (ms * 1e-3) / 1e9}
+        # f4 on the same atmospheres: stored coefficients, one source species, 2 048 columns
+        ncol, ld, nr = 2048, atm.ld, net.n_reactions
+        kf = torch.empty((nr, ld), dtype=torch.float64, device="cuda")
+        kr = torch.empty_like(kf)
+        h.rate_coeffs(ncol, ld, dev(atm.T), dev(atm.P), dev(atm.J), kf, kr, ws_for(h.rate_coeffs_workspace_bytes(ncol)))
+        dist = torch.empty((net.n_species, ld), dtype=torch.float64, device="cuda")
+        pred = torch.empty((net.n_species, ld), dtype=torch.int32, device="cuda")
+        via = torch.empty_like(pred)
+        ws = ws_for(h.pathway_workspace_bytes(ncol))
+        call = lambda: h.pathway(ncol, ld, kf, kr, args[0], 0, dist, pred, via, ws)
+        call()
+        sync()
+        h.tune(binding.XOD_TUNE_TIMING, 1)
+        ms = event_time_ms(call, 3, sync)
+        kt = h.timing_read()
+        h.tune(binding.XOD_TUNE_TIMING, 0)
+        out["f4_pathway"] = {"ncol": ncol, "ms": ms, "columns_per_s": ncol / (ms * 1e-3), "kernel_ms": {k: v[0] / 3 for k, v in kt.items() if v[1]}}
+        h.close()
+    except Exception as exc:
+        out["f3_f4"] = {"error": repr(exc)[:300]}
     return out
 
 
@@ -415,7 +446,7 @@ def run_ours(args):
 
     T, P, J, n = dev(atm.T), dev(atm.P), dev(atm.J), dev(atm.n)
     dndt = torch.empty((ns, ld), dtype=torch.float64, device="cuda")
-    ws = torch.empty(h.source_fused_workspace_bytes(ncol) // 8 + 64, dtype=torch.float64, device="cuda")
+    ws = torch.empty(h.source_fused_workspace_bytes(ncol, prod_loss=False) // 8 + 64, dtype=torch.float64, device="cuda")
     step = lambda: h.source_fused(ncol, ld, T, P, J, n, dndt, workspace=ws)
 
     def barrier():

@@ -182,12 +182,16 @@ xod_status xod_rate_coeffs(const xod_network *net, int64_t ncol, int64_t ld, con
  * memory owned by the caller; workspace >= xod_source_workspace_bytes(net, ncol).
  * Errors: XOD_ERR_INVALID_ARG, XOD_ERR_WORKSPACE, XOD_ERR_CUDA. */
 size_t xod_source_workspace_bytes(const xod_network *net, int64_t ncol);
+/* the (much smaller) requirement when prod and loss are NULL: only the partial sums of the single-kernel path */
+size_t xod_source_workspace_bytes_dndt(const xod_network *net, int64_t ncol);
 xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
                       const double *kr, const double *n, double *dndt, double *prod, double *loss,
                       void *workspace, size_t workspace_bytes, void *stream);
 
 /* ---- a1-a8 fused: (T, P, J, n) -> dn/dt without k_f, k_r ever reaching HBM (the headline path). */
 size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol);
+/* the requirement when prod and loss are NULL (0-few MB instead of the multi-kernel scratch of the P/L variant) */
+size_t xod_source_fused_workspace_bytes_dndt(const xod_network *net, int64_t ncol);
 xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
                             const double *P, const double *J, const double *n, double *dndt,
                             double *prod, double *loss, void *workspace, size_t workspace_bytes,

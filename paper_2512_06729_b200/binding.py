@@ -30,7 +30,8 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_check_status", "xod_build_has_checks", "xod_network_jac_info", "xod_network_lu_info", "xod_network_lu_pattern",
            "xod_newton_workspace_bytes", "xod_newton_step", "xod_photo_create", "xod_photo_destroy",
            "xod_photo_workspace_bytes", "xod_photo_rates", "xod_transport",
-           "xod_pathway_workspace_bytes", "xod_pathway"]
+           "xod_pathway_workspace_bytes", "xod_pathway",
+           "xod_source_workspace_bytes_dndt", "xod_source_fused_workspace_bytes_dndt"]
 
 
 class XodError(RuntimeError):
@@ -58,7 +59,8 @@ def lib():
         L = C.CDLL(_LIB_PATH)
         L.xod_last_error.restype = C.c_char_p
         for name in ("xod_rate_coeffs_workspace_bytes", "xod_source_workspace_bytes",
-                     "xod_source_fused_workspace_bytes", "xod_newton_workspace_bytes", "xod_pathway_workspace_bytes"):
+                     "xod_source_fused_workspace_bytes", "xod_newton_workspace_bytes", "xod_pathway_workspace_bytes",
+                     "xod_source_workspace_bytes_dndt", "xod_source_fused_workspace_bytes_dndt"):
             getattr(L, name).restype = C.c_size_t
             getattr(L, name).argtypes = [C.c_void_p, C.c_int64]
         L.xod_photo_workspace_bytes.restype = C.c_size_t
@@ -212,11 +214,14 @@ class Network:
     def rate_coeffs_workspace_bytes(self, ncol):
         return lib().xod_rate_coeffs_workspace_bytes(self._h, ncol)
 
-    def source_workspace_bytes(self, ncol):
-        return lib().xod_source_workspace_bytes(self._h, ncol)
+    def source_workspace_bytes(self, ncol, prod_loss=True):
+        f = lib().xod_source_workspace_bytes if prod_loss else lib().xod_source_workspace_bytes_dndt
+        return f(self._h, ncol)
 
-    def source_fused_workspace_bytes(self, ncol):
-        return lib().xod_source_fused_workspace_bytes(self._h, ncol)
+    def source_fused_workspace_bytes(self, ncol, prod_loss=True):
+        """Upper bound for any arguments; prod_loss=False: the requirement when prod and loss are not asked for."""
+        f = lib().xod_source_fused_workspace_bytes if prod_loss else lib().xod_source_fused_workspace_bytes_dndt
+        return f(self._h, ncol)
 
     # ---- compute calls (device tensors)
     def thermo(self, ncol, ld, T, cp_R=None, h_RT=None, s_R=None, g_RT=None, stream=None):

@@ -648,6 +648,12 @@ size_t xod_source_workspace_bytes(const xod_network *net, int64_t ncol) {
   return std::max(scratch_bytes(net, chunk_cols(net, ncol), false, true, true), fused_partial_bytes(net, ncol));
 }
 
+size_t xod_source_workspace_bytes_dndt(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0) return 0;
+  if (net->fd.enabled && net->use_fused && net->h.nr > 0) return fused_partial_bytes(net, ncol) + 16;
+  return scratch_bytes(net, chunk_cols(net, ncol), false, true, false);
+}
+
 xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const double *kf,
                       const double *kr, const double *n, double *dndt, double *prod, double *loss,
                       void *workspace, size_t workspace_bytes, void *stream) {
@@ -657,10 +663,10 @@ xod_status xod_source(const xod_network *net, int64_t ncol, int64_t ld, const do
   if (!n || !dndt) return fail(XOD_ERR_INVALID_ARG, "n or dndt is NULL");
   if (net->h.nr > 0 && (!kf || !kr)) return fail(XOD_ERR_INVALID_ARG, "kf or kr is NULL");
   if ((prod == nullptr) != (loss == nullptr)) return fail(XOD_ERR_INVALID_ARG, "prod and loss must be given together");
-  if (!workspace || workspace_bytes < xod_source_workspace_bytes(net, ncol))
-    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_workspace_bytes");
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
   const bool pl = prod != nullptr;
+  if (!workspace || workspace_bytes < (pl ? xod_source_workspace_bytes(net, ncol) : xod_source_workspace_bytes_dndt(net, ncol)))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_workspace_bytes (xod_source_workspace_bytes_dndt without prod/loss)");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (!pl && net->fd.enabled && net->use_fused && net->h.nr > 0)
     return launch_fused(net, ncol, ld, nullptr, nullptr, nullptr, kf, kr, n, dndt, workspace, s);
   const int64_t ldw = chunk_cols(net, ncol);
@@ -690,6 +696,12 @@ size_t xod_source_fused_workspace_bytes(const xod_network *net, int64_t ncol) {
   return std::max(scratch_bytes(net, chunk_cols(net, ncol), true, true, true), fused_partial_bytes(net, ncol));
 }
 
+size_t xod_source_fused_workspace_bytes_dndt(const xod_network *net, int64_t ncol) {
+  if (!net || ncol < 0) return 0;
+  if (net->fd.enabled && net->use_fused) return fused_partial_bytes(net, ncol) + 16;
+  return scratch_bytes(net, chunk_cols(net, ncol), true, true, false);
+}
+
 xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, const double *T,
                             const double *P, const double *J, const double *n, double *dndt,
                             double *prod, double *loss, void *workspace, size_t workspace_bytes,
@@ -700,10 +712,10 @@ xod_status xod_source_fused(const xod_network *net, int64_t ncol, int64_t ld, co
   if (!T || !P || !n || !dndt) return fail(XOD_ERR_INVALID_ARG, "T, P, n or dndt is NULL");
   if (net->h.n_photo > 0 && !J) return fail(XOD_ERR_INVALID_ARG, "J is NULL but the network has photolysis reactions");
   if ((prod == nullptr) != (loss == nullptr)) return fail(XOD_ERR_INVALID_ARG, "prod and loss must be given together");
-  if (!workspace || workspace_bytes < xod_source_fused_workspace_bytes(net, ncol))
-    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_fused_workspace_bytes");
-  cudaStream_t s = static_cast<cudaStream_t>(stream);
   const bool pl = prod != nullptr;
+  if (!workspace || workspace_bytes < (pl ? xod_source_fused_workspace_bytes(net, ncol) : xod_source_fused_workspace_bytes_dndt(net, ncol)))
+    return fail(XOD_ERR_WORKSPACE, "workspace NULL or smaller than xod_source_fused_workspace_bytes (xod_source_fused_workspace_bytes_dndt without prod/loss)");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (!pl && net->fd.enabled && net->use_fused)
     return launch_fused(net, ncol, ld, T, P, J, nullptr, nullptr, n, dndt, workspace, s);
   const int64_t ldw = chunk_cols(net, ncol);
@@ -765,8 +777,8 @@ xod_status xod_source_fused_host(xod_network *net, int64_t ncol, int64_t ld, con
   const size_t ns = net->h.ns, nph = net->h.n_photo;
   const int64_t cw = std::min<int64_t>(round_up(ncol, 32), (int64_t)net->sm_count * kFW);  // columns per chunk
   // the ragged last chunk runs with fewer tiles and therefore more reaction splits: size for both widths
-  const size_t ws = std::max(xod_source_fused_workspace_bytes(net, cw),
-                             ncol % cw ? xod_source_fused_workspace_bytes(net, ncol % cw) : 0) + 256;
+  const size_t ws = std::max(xod_source_fused_workspace_bytes_dndt(net, cw),
+                             ncol % cw ? xod_source_fused_workspace_bytes_dndt(net, ncol % cw) : 0) + 256;
   const size_t rows = 2 + nph + 2 * ns;
   const size_t slot_bytes = round_up((int64_t)(rows * cw * sizeof(double) + ws), 256);
   const size_t need = slot_bytes * kHostSlots;
@@ -849,7 +861,10 @@ size_t xod_newton_workspace_bytes(const xod_network *net, int64_t ncol) {
   if (!net || ncol < 0 || !net->h.lu.enabled) return 0;
   const int64_t cw = newton_chunk(ncol);
   const size_t rows = (size_t)2 * net->h.ns + (size_t)net->h.jac_col.size() + (size_t)net->h.lu.nnz;
-  return rows * (size_t)cw * sizeof(double) + fused_partial_bytes(net, cw) + 1024;
+  // k_fused's partial sums: a narrower last pass has fewer tiles, hence more reaction splits and a larger buffer
+  const int64_t last = ncol % cw;
+  const size_t part = std::max(ncol >= cw ? fused_partial_bytes(net, cw) : 0, last ? fused_partial_bytes(net, last) : 0);
+  return rows * (size_t)cw * sizeof(double) + part + 1024;
 }
 
 xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,

@@ -359,6 +359,17 @@ delta1 = np.zeros_like(y1)
 dt1 = np.full(atm1.ld, 1e-3)
 assert emu.emu_newton_step(C.byref(d1), C.c_int64(atm1.ncol), C.c_int64(atm1.ld), tk.ptr(k1), tk.ptr(k1), tk.ptr(atm1.n),
                            tk.ptr(dt1), tk.ptr(y1), tk.ptr(delta1)) == 0
+# the pathway analyser: double-buffered distance tiles, partial minima combined after a barrier, __syncthreads_or
+dist1 = np.zeros_like(y1)
+pred1, via1 = np.zeros(y1.shape, dtype=np.int32), np.zeros(y1.shape, dtype=np.int32)
+assert emu.emu_pathway(C.byref(d1), C.c_int64(atm1.ncol), C.c_int64(atm1.ld), tk.ptr(k1), tk.ptr(k1), tk.ptr(atm1.n), C.c_int(2),
+                       tk.ptr(dist1), tk.ptr(pred1), tk.ptr(via1), C.c_int(2)) == 0
+# the photolysis contraction: shared operand tiles of the GEMM, the scan tile of k_photo_flux
+import test_photo_rates as tp
+tk.LIB = sys.argv[2]
+atm3 = synth.config_atmosphere(1, net1, 2)
+ph = synth.make_photo(51, net1, n_bins=70)
+tp.run_emulated(net1, atm3, ph, *synth.make_irradiation(52, net1, atm3, ph))
 print("emulated-ok")
 """
 
@@ -399,6 +410,15 @@ net = synth.config_network(1)
 atm = synth.config_atmosphere(1, net, 3)
 ph = synth.make_photo(51, net, n_bins=70)
 tp.run_emulated(net, atm, ph, *synth.make_irradiation(52, net, atm, ph))
+t = synth.make_transport(61, net, atm)
+arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (atm.n, atm.T, t["n_gas"], t["D"], t["mass"], t["alpha_T"], t["mbar"], t["grav"], t["dz"])]
+tr = np.zeros((net.n_species, atm.ld))
+assert emu.emu_transport(C.c_int(net.n_species), C.c_int64(3), C.c_int64(20), C.c_int64(atm.ld), *[tk.ptr(x) for x in arrs], tk.ptr(tr), C.c_int(5)) == 0
+import test_pathway as tpw
+net2 = synth.config_network(2)
+atm2 = synth.config_atmosphere(2, net2)
+k2 = np.full((net2.n_reactions, atm2.ld), 1e-12)
+tpw.run_emulated(net2, k2, k2, atm2.n, 37, atm2.ld, 5, 2)
 print("emulated-ok")
 """
 
@@ -424,7 +444,7 @@ def test_kernel_sources_touch_no_memory_outside_their_buffers_under_address_sani
 def test_barrier_synchronised_kernel_sources_are_race_free_under_thread_sanitizer():
     """racecheck substitute (compute-sanitizer is closed on the GPU pool): the emulated CUDA threads are
     real threads and __syncthreads a real barrier, so ThreadSanitizer sees every shared-memory access
-    of k_fused, k_jac_tiled and k_lu_factor between barriers: the double-buffered values and schedule, the accumulator
+    of k_fused, k_jac_tiled, k_lu_factor, k_pathway, k_photo_gemm and k_photo_flux between barriers: the double-buffered values and schedule, the accumulator
     read-modify-writes of the row tasks, the per-unit flush, the tile prologue/epilogue.  (Removing the per-chunk barrier makes it report.)"""
     tsan = subprocess.run(["gcc", "-print-file-name=libtsan.so"], capture_output=True, text=True).stdout.strip()
     if not os.path.isabs(tsan) or not os.path.exists(tsan):
