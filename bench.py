@@ -532,7 +532,10 @@ def run_ours(args):
     stages = None
     if not args.no_stages:
         del hT, hP, hJ, hn, hd
-        stages = stage_timings(binding, h, net, dev, lambda b: torch.empty(b // 8 + 64, dtype=torch.float64, device="cuda"), dfma)
+        try:
+            stages = stage_timings(binding, h, net, dev, lambda b: torch.empty(b // 8 + 64, dtype=torch.float64, device="cuda"), dfma)
+        except Exception as exc:      # a failing stage must not cost the headline line
+            stages = {"error": repr(exc)[:300]}
     cpu = None
     if not args.no_cpu_baseline:
         cpu, _, _ = oracle_throughput(net, atm, atm.meta["n_layers"], target_s=10.0)

@@ -118,6 +118,7 @@ xod_status xod_network_fused_info(const xod_network *net, int64_t *info);
  *   log2 k_f (or log2 k_inf) = c0 + c1 log2 T + c2/T                                        (Eq. 7, 11)
  *   C0 + C1 log2 T + C2/T - T (D2 + T (D3 + T (D4 + T D5))) = log2 k_r (UNI/BI) or log2 (k_r/k_f) (FALLOFF)
  *   log2 k0 = l0 + l1 log2 T + l2/T                                                           (Eq. 10)
+ * An irreversible reaction or a padding slot is reported with C0 = -inf (k_r = 0).
  * breakpoints [info[4]]: the sorted distinct t_mid values; a column with T is in interval #{bp < T}.
  * Any output may be NULL. */
 xod_status xod_network_fused_params(const xod_network *net, int32_t interval, int32_t *user_rxn, int32_t *kind,

@@ -394,6 +394,11 @@ xod_status xod_network_fused_params(const xod_network *net, int32_t interval, in
     const unsigned char *blk = &f.blk[(size_t)interval * f.blk_stride + off + (size_t)((pp - first) / kFRxnPerWarp) * bsz];
     const int slot = (pp - first) % kFRxnPerWarp, npair = seg == 0 ? 5 : 8;
     for (int u = 0; u < npair; ++u) std::memcpy(out + 2 * u, blk + (2 + u) * 64 + slot * 16, 16);
+    // an irreversible reaction (or a padding slot) has k_r = 0: the blocks hold zeros there and the kernels select 0
+    // by the reversible flag / the zeros row of the n tile; this view reports the equivalent C0 = -inf
+    int32_t u1[4];
+    std::memcpy(u1, blk + 64 + slot * 16, 16);
+    if (!(u1[3] & 1)) out[3] = -INFINITY;
   }
   return XOD_OK;
 }

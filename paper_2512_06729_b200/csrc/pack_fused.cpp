@@ -40,9 +40,9 @@ void scaled_nasa(const double *a, long double b[7]) {
 }  // namespace
 
 size_t fused_smem_bytes(int ns, int n_acc, int chunk, int meta_cap) {
-  // n tile (+ ones row) | accumulator rows | two q buffers (+ zero row each) | two chunk schedules
-  // | column scalars
-  return ((size_t)(ns + 1) + (size_t)n_acc + 2 * (size_t)(chunk + 1)) * kFW * sizeof(double) +
+  // n tile (+ ones row, zeros row) | accumulator rows | two q buffers (+ zero row each) | two chunk
+  // schedules | column scalars
+  return ((size_t)(ns + 2) + (size_t)n_acc + 2 * (size_t)(chunk + 1)) * kFW * sizeof(double) +
          2 * (size_t)meta_cap * 16 + (size_t)kFW * (4 * sizeof(double) + sizeof(int32_t));
 }
 
@@ -130,7 +130,9 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
   //   reverse coefficients, per interval (seven numbers per reaction):
   //   UNI/BI : C0 = c0 + dB0, C1 = c1 - dB1, C2 = c2 + dB6   (k_f folded in: one exp2 gives k_r)
   //   FALLOFF: C0 = dB0, C1 = -dB1, C2 = dB6                 (pure z; added to log2 k_f in the kernel)
-  //   irreversible, padding: C0 = -inf, rest 0               (k_r = 0)
+  //   irreversible: all seven 0 (k_r = 1 or k_f, finite) and the first product slot points at the zeros row of
+  //   the n tile, so q_r = 0 exactly without a special case on the kernel's fast path; k_rate_coeffs, which
+  //   stores k_r itself, selects 0 by the reversible flag (word 3 of unit 1).  Padding slots: all 0, ones rows.
   const int ng = f.n_bp + 1;
   const int64_t n_arr_g = f.arr_end / kFRxnPerWarp, n_fo_g = (f.fo_end - f.arr_end) / kFRxnPerWarp,
                 n_ph_g = (f.ph_end - f.fo_end) / kFRxnPerWarp;
@@ -153,11 +155,12 @@ void pack_fused(const xod_network_desc *d, HostTables &h, int chunk) {
       const int slot = (pp - first) % kFRxnPerWarp;
       const int p = f.pp_to_packed[pp];
       int32_t sp8[8] = {ns, ns, ns, ns, ns, ns, 0, 0};  // absent species -> the ones row of the n tile
-      double v[16] = {0, 0, 0, -INFINITY, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      double v[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
       if (p >= 0) {
         for (int a = 0; a < 6; ++a)
           if (h.sp[(size_t)p * 6 + a] >= 0) sp8[a] = h.sp[(size_t)p * 6 + a];
         sp8[7] = h.flags[p];
+        if (p < h.ph_begin && !(h.flags[p] & 1)) sp8[3] = ns + 1, sp8[4] = ns, sp8[5] = ns;   // irreversible: zeros row
         if (p >= h.ph_begin) sp8[6] = h.photo_row[p - h.ph_begin];
         v[0] = h.c0[p], v[1] = h.c1[p], v[2] = h.c2[p];
         if (p < h.ph_begin && (h.flags[p] & 1)) {
@@ -343,9 +346,16 @@ bool check_fused(const HostTables &h, std::string &err) {
       const int p = f.pp_to_packed[pp];
       const int slots[6] = {u[0] & 0xffff, (int)((uint32_t)u[0] >> 16), u[1] & 0xffff, (int)((uint32_t)u[1] >> 16),
                             u[2] & 0xffff, (int)((uint32_t)u[2] >> 16)};
+      const bool irrev = p >= 0 && p < h.ph_begin && !(h.flags[p] & 1);   // products: zeros row, ones, ones
       for (int a = 0; a < 6; ++a) {
-        const int expect = p >= 0 && h.sp[(size_t)p * 6 + a] >= 0 ? h.sp[(size_t)p * 6 + a] : ns;
+        int expect = p >= 0 && h.sp[(size_t)p * 6 + a] >= 0 ? h.sp[(size_t)p * 6 + a] : ns;
+        if (irrev && a >= 3) expect = a == 3 ? ns + 1 : ns;
         if (slots[a] != expect) return fail("species slot mismatch in a parameter block");
+      }
+      {
+        int32_t u1[4];
+        std::memcpy(u1, blk + 64 + ((pp - first) % kFRxnPerWarp) * 16, 16);
+        if (p >= 0 && u1[3] != h.flags[p]) return fail("reversible flag mismatch in a parameter block");
       }
       if (p >= h.ph_begin && u[3] != h.photo_row[p - h.ph_begin]) return fail("J row mismatch in a parameter block");
       if (u[3] < 0 || (h.n_photo > 0 && u[3] >= h.n_photo) ) return fail("J row out of range");

@@ -50,9 +50,10 @@ __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, i
       const double y = fma(c2C.x, iT, fma(c01.y, l2T, c01.x));
       const double poly = fma(Tc, fma(Tc, fma(Tc, d45.y, d45.x), d23.y), d23.x);
       const double z = fma(c12.y, iT, fma(c12.x, l2T, fma(-Tc, poly, c2C.y)));
+      const bool rev = __ldg(reinterpret_cast<const int *>(b + 64) + 3) & 1;   // irreversible: k_r = 0 (the blocks hold z = 0)
       if (arr) {
         vf = xexp2(y);
-        vr = xexp2(z);
+        vr = rev ? xexp2(z) : 0.0;
       } else {
         const double2 m01 = __ldg(reinterpret_cast<const double2 *>(b + 7 * 64));
         const double2 m2f = __ldg(reinterpret_cast<const double2 *>(b + 8 * 64));
@@ -63,7 +64,7 @@ __global__ void __launch_bounds__(256) k_rate_coeffs(FusedDev f, int64_t ncol, i
         const double den = 1.0 / (1.0 + xexp2(-fabs(lp)));
         const double ym = fmin(w, y) + lF;
         vf = xexp2(ym) * den;
-        vr = xexp2(ym + z) * den;
+        vr = rev ? xexp2(ym + z) * den : 0.0;
       }
     } else {
       const unsigned char *b = blkg + XOD_IDX((size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh, (size_t)f.blk_stride) + slot16;

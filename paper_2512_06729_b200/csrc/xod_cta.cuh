@@ -20,6 +20,39 @@ __device__ __forceinline__ void cp_async8(void *smem, const void *gmem) {
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 
+// ---- explicit shared-memory accesses by 32-bit address in the CTA's shared window.  The scheduled row
+// reduction (sched.cuh) lives entirely in shared memory; with plain pointers the compiler rebuilt generic
+// addresses (window base, kernel parameters) inside its inner loops.  ld/st.shared on an address register
+// leaves it nothing to rematerialise.
+typedef unsigned smem_addr;
+// an opaque "mov r, r": the value now comes out of an instruction the compiler cannot recompute elsewhere, so a
+// loop invariant stays in its register instead of being rebuilt from the thread index and kernel parameters
+#define XOD_KEEP(r) asm volatile("mov.b32 %0, %0;\n" : "+r"(r))
+__device__ __forceinline__ smem_addr smem_addr_of(const void *p) { return (smem_addr)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned lds_u32(smem_addr a) {
+  unsigned v;
+  asm volatile("ld.shared.u32 %0, [%1];\n" : "=r"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned lds_u16(smem_addr a) {
+  unsigned short v;
+  asm volatile("ld.shared.u16 %0, [%1];\n" : "=h"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ int2 lds_i2(smem_addr a) {
+  int2 v;
+  asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];\n" : "=r"(v.x), "=r"(v.y) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ double2 lds_d2(smem_addr a) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];\n" : "=d"(v.x), "=d"(v.y) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts_d2(smem_addr a, double2 v) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};\n" ::"r"(a), "d"(v.x), "d"(v.y) : "memory");
+}
+
 // ---- XOD_IDX(i, n): a table-derived index i that must lie in [0, n).
 // Default build: the identity (no code).  -DXOD_CHECK build (debugging only, `XOD_CHECK=1 python -m
 // paper_2512_06729_b200.build`): an out-of-range index records the source line in a device flag

@@ -18,7 +18,7 @@
 #define __launch_bounds__(...)
 #define __align__(n) __attribute__((aligned(n)))
 
-struct int2 { int x, y; };
+struct alignas(8) int2 { int x, y; };
 struct alignas(16) int4 { int x, y, z, w; };
 struct uint2 { unsigned x, y; };
 struct alignas(16) double2 { double x, y; };
