@@ -245,3 +245,22 @@ class Oracle:
                                   _ptr(dist), _ptr(pred), _ptr(via))
         assert rc == 0
         return dist, pred, via
+
+    # ---- f4: thermochemical-equilibrium composition
+    def equilibrium(self, net, T, P, b, ncol=None, max_iter=2000, tol=1e-15, want_pi=False):
+        """n [n_species][ld] minimising the Gibbs energy at (T, P) for element abundances b [n_elements][ld];
+        also the iterations used per column (negative: not converged) and, on request, the element potentials."""
+        T, P, b = _f64(T), _f64(P), _f64(b)
+        ld = b.shape[1]
+        ncol = ld if ncol is None else ncol
+        ns, _ = self._dims(net)
+        ne = np.asarray(net.composition).shape[1]
+        s, keep = self._net(net)
+        n = np.full((ns, ld), np.nan)
+        pi = np.full((ne, ld), np.nan)
+        iters = np.zeros(ld, dtype=np.int32)
+        rc = self.lib.orc_equilibrium(C.byref(s), C.c_long(ncol), C.c_long(ld), _ptr(T), _ptr(P), _ptr(b), C.c_int(max_iter),
+                                      C.c_double(tol), _ptr(n), _ptr(pi), _ptr(iters))
+        if rc != 0:
+            raise ArithmeticError("oracle equilibrium failed (%d: -2 singular system, -3 element without abundance)" % rc)
+        return (n, iters, pi) if want_pi else (n, iters)

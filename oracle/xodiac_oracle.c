@@ -706,3 +706,147 @@ int orc_pathway(const orc_network *net, long ncol, long ld, const double *kf, co
   free(pred);
   return 0;
 }
+
+/* ---------------------------------------------------------------- f4: thermochemical-equilibrium composition
+ * PAPER.md:248 (section 2.5): "the initial atmospheric composition can be specified using ... (i) equilibrium
+ * abundances from the built-in equilibrium chemistry solver NEXOCHEM"; a Gibbs-energy
+ * minimisation that reuses the NASA-7 thermochemistry.  The paper names the solver and gives no method, so the
+ * oracle computes the DEFINITION (reading E1): for a column at (T, P) with element abundances b_e, the
+ * equilibrium composition of an ideal gas mixture is the n >= 0 that minimises
+ *     G / RT = sum_i n_i ( G_i/RT (T) + ln (n_i / N) + ln (P / P0) ),   N = sum_i n_i,
+ * subject to sum_i a_ie n_i = b_e for every element e (a_ie = the composition matrix; a column of it with entries of
+ * both signs is the charge, b = 0 for a neutral gas).  Only the ratios of b matter; the result is returned as number
+ * densities n_i = x_i P / (k_B T), x_i = n_i / N.  G is strictly convex on the feasible set, so the minimiser is
+ * unique and is characterised by the Lagrange conditions
+ *     G_i/RT + ln x_i + ln (P / P0) = sum_e a_ie pi_e  for every species,   sum_i x_i = 1,   sum_i a_ie x_i  ~  b_e,
+ * pi_e = the element potentials (over RT).  These are also exactly the conditions under which every reversible
+ * reaction of the kinetics has q_f = q_r (O3: K_c from the same G_i/RT), i.e. dn/dt = 0 without photolysis.
+ * Method: the Lagrange conditions are solved by the damped Newton iteration of Gordon & McBride (NASA RP-1311, 1994,
+ * section 2.3, gas phase only): unknowns ln n_i, ln N; each iteration solves the (n_e + 1) x (n_e + 1) system
+ *     sum_e' ( sum_i a_ie a_ie' n_i ) pi_e' + ( sum_i a_ie n_i ) dlnN = b_e - sum_i a_ie n_i + sum_i a_ie n_i mu_i
+ *     sum_e' ( sum_i a_ie' n_i ) pi_e'      + ( sum_i n_i - N ) dlnN  = N - sum_i n_i + sum_i n_i mu_i
+ * with mu_i = G_i/RT + ln (n_i / N) + ln (P / P0), then dln n_i = -mu_i + sum_e a_ie pi_e + dlnN, and applies
+ * lambda = min(1, 2 / max(5 |dlnN|, max over species with ln (n_i/N) > -18.42 of |dln n_i|),
+ *              min over the other species with dln n_i > 0 of |(-ln (n_i/N) - 9.21) / (dln n_i - dlnN)|)
+ * of the step.  Start: b scaled to sum 1, N = 0.1, n_i = 0.1 / n_species.  Converged when lambda = 1,
+ * max_i n_i |dln n_i| / sum n <= tol, N |dlnN| / sum n <= tol and |sum_i a_ie n_i - b_e| <= tol max b for every e;
+ * then ln n_i = ln N + sum_e a_ie pi_e - G_i/RT - ln (P / P0) is taken for EVERY species (trace species sit exactly
+ * on the Lagrange condition).  The linear system is solved by Gaussian elimination with partial pivoting after each
+ * row is divided by its largest entry (a charge row is many orders below the element rows).  Plain loops, one
+ * column at a time, real_t arithmetic.
+ * Outputs: n [n_species][ld]; pi (optional) [n_elements][ld]; iters (optional) [ld] = iterations used, negated if
+ * max_iter was reached first.  Returns 0, -1 (memory), -2 (singular system), -3 (an element with b_e <= 0 whose
+ * composition column has no negative entry).
+ * Pins (tests/test_oracle_equilibrium.py): A <=> B and A2 <=> 2 A in closed form; the Lagrange conditions rebuilt by
+ * the test from orc_thermo (least squares over pi); element conservation and sum x = 1; the kinetic fixed point
+ * (orc_source gives dn/dt = 0 at the returned composition when J = 0); G at the returned composition below G at
+ * feasible perturbations; invariance under scaling b; a pressure shift moves A2 <=> 2 A the Le Chatelier way. */
+static int solve_scaled_real(long n, real_t *A, real_t *b, real_t *x) {
+  for (long i = 0; i < n; ++i) {
+    real_t m = 0;
+    for (long j = 0; j < n; ++j)
+      if (R_FABS(A[i * n + j]) > m) m = R_FABS(A[i * n + j]);
+    if (m == 0) return -1;
+    for (long j = 0; j < n; ++j) A[i * n + j] /= m;
+    b[i] /= m;
+  }
+  return solve_dense_real(n, A, b, x);
+}
+
+int orc_equilibrium(const orc_network *net, long ncol, long ld, const double *T, const double *P, const double *b_in,
+                    int max_iter, double tol, double *n_out, double *pi_out, int *iters_out) {
+  const int ns = net->n_species, ne = net->n_elements, m = ne + 1;
+  real_t *lnn = (real_t *)malloc(sizeof(real_t) * (size_t)(4 * ns + 2 * m + 2 * m * m + ne));
+  if (!lnn) return -1;
+  real_t *c = lnn + ns, *dln = c + ns, *nn = dln + ns, *M = nn + ns, *rhs = M + m * m, *sol = rhs + m, *b = sol + m;
+  int rc = 0;
+  for (long col = 0; col < ncol && rc == 0; ++col) {
+    const real_t Tc = (real_t)T[col], lnP = R_LOG((real_t)P[col] / P_REF);
+    real_t bsum = 0, bmax = 0;
+    for (int e = 0; e < ne; ++e) {
+      b[e] = (real_t)b_in[(long)e * ld + col];
+      int has_neg = 0;
+      for (int i = 0; i < ns; ++i) has_neg |= net->composition[i * ne + e] < 0;
+      if (!(b[e] > 0) && !has_neg) rc = -3;
+      if (b[e] > 0) bsum += b[e];
+    }
+    if (rc != 0) break;
+    for (int e = 0; e < ne; ++e) {
+      b[e] /= bsum;
+      if (R_FABS(b[e]) > bmax) bmax = R_FABS(b[e]);
+    }
+    for (int i = 0; i < ns; ++i) {
+      c[i] = nasa_g(nasa_set(net, i, Tc), Tc) + lnP;
+      lnn[i] = R_LOG((real_t)0.1 / (real_t)ns);
+    }
+    real_t lnN = R_LOG((real_t)0.1);
+    int it = 0, done = 0;
+    while (!done && it < max_iter) {
+      ++it;
+      const real_t N = R_EXP(lnN);
+      for (int k = 0; k < m * m; ++k) M[k] = 0;
+      for (int k = 0; k < m; ++k) rhs[k] = 0;
+      real_t sumn = 0, sumnmu = 0;
+      for (int i = 0; i < ns; ++i) {
+        const real_t ni = R_EXP(lnn[i]), mu = c[i] + lnn[i] - lnN;
+        nn[i] = ni;
+        sumn += ni, sumnmu += ni * mu;
+        for (int e = 0; e < ne; ++e) {
+          const real_t ae = (real_t)net->composition[i * ne + e];
+          if (ae == 0) continue;
+          for (int f = 0; f < ne; ++f) M[e * m + f] += ae * (real_t)net->composition[i * ne + f] * ni;
+          M[e * m + ne] += ae * ni;
+          M[ne * m + e] += ae * ni;
+          rhs[e] += ae * ni * mu;
+        }
+      }
+      for (int e = 0; e < ne; ++e) rhs[e] += b[e] - M[e * m + ne];
+      M[ne * m + ne] = sumn - N;
+      rhs[ne] = N - sumn + sumnmu;
+      if (solve_scaled_real(m, M, rhs, sol) != 0) { rc = -2; break; }
+      const real_t dlnN = sol[ne];
+      real_t big = 5 * R_FABS(dlnN), lam2 = 1;
+      for (int i = 0; i < ns; ++i) {
+        real_t d = -(c[i] + lnn[i] - lnN) + dlnN;
+        for (int e = 0; e < ne; ++e) d += (real_t)net->composition[i * ne + e] * sol[e];
+        dln[i] = d;
+        const real_t lx = lnn[i] - lnN;
+        if (lx > (real_t)-18.420681L) {
+          if (R_FABS(d) > big) big = R_FABS(d);
+        } else if (d > 0) {
+          const real_t l = R_FABS((-lx - (real_t)9.2103404L) / (d - dlnN));
+          if (l < lam2) lam2 = l;
+        }
+      }
+      real_t lam = big > 2 ? 2 / big : 1;
+      if (lam2 < lam) lam = lam2;
+      real_t err = 0, newsum = 0;
+      for (int i = 0; i < ns; ++i) lnn[i] += lam * dln[i], newsum += R_EXP(lnn[i]);
+      lnN += lam * dlnN;
+      for (int i = 0; i < ns; ++i) {
+        const real_t w = R_EXP(lnn[i]) * R_FABS(dln[i]) / newsum;
+        if (w > err) err = w;
+      }
+      if (R_EXP(lnN) * R_FABS(dlnN) / newsum > err) err = R_EXP(lnN) * R_FABS(dlnN) / newsum;
+      real_t res = 0;
+      for (int e = 0; e < ne; ++e) {
+        real_t s = -b[e];
+        for (int i = 0; i < ns; ++i) s += (real_t)net->composition[i * ne + e] * R_EXP(lnn[i]);
+        if (R_FABS(s) > res) res = R_FABS(s);
+      }
+      done = lam == 1 && err <= (real_t)tol && res <= (real_t)tol * bmax;
+    }
+    if (rc != 0) break;
+    const real_t ntot = (real_t)P[col] / (K_BOLTZ * Tc);
+    for (int i = 0; i < ns; ++i) {
+      real_t lx = -c[i];   /* ln x_i = sum_e a_ie pi_e - G_i/RT - ln (P/P0), every species on the Lagrange condition */
+      for (int e = 0; e < ne; ++e) lx += (real_t)net->composition[i * ne + e] * sol[e];
+      n_out[(long)i * ld + col] = (double)(ntot * R_EXP(lx));
+    }
+    if (pi_out)
+      for (int e = 0; e < ne; ++e) pi_out[(long)e * ld + col] = (double)sol[e];
+    if (iters_out) iters_out[col] = done ? it : -it;
+  }
+  free(lnn);
+  return rc;
+}
