@@ -416,6 +416,18 @@ def next_row_timings(binding, net, dev, ws_for):
         kt = h.timing_read()
         h.tune(binding.XOD_TUNE_TIMING, 0)
         out["f4_pathway"] = {"ncol": ncol, "ms": ms, "columns_per_s": ncol / (ms * 1e-3), "kernel_ms": {k: v[0] / 3 for k, v in kt.items() if v[1]}}
+        # f4 equilibrium start: the same 2 048 columns, element abundances of the synthetic composition
+        comp = np.asarray(net.composition, dtype=np.float64)
+        b = dev(comp.T @ atm.n)
+        neq = torch.empty((net.n_species, ld), dtype=torch.float64, device="cuda")
+        iters = torch.zeros((ld,), dtype=torch.int32, device="cuda")
+        call = lambda: h.equilibrium(ncol, ld, dev(atm.T), dev(atm.P), b, neq, None, iters)
+        call()
+        sync()
+        ms = event_time_ms(call, 3, sync)
+        itn = iters[:ncol].cpu().numpy()
+        out["f4_equilibrium"] = {"ncol": ncol, "ms": ms, "columns_per_s": ncol / (ms * 1e-3), "converged": int((itn > 0).sum()),
+                                 "iterations_max": int(abs(itn).max())}
         h.close()
     except Exception as exc:
         out["f3_f4"] = {"error": repr(exc)[:300]}

@@ -299,13 +299,35 @@ xod_status xod_transport(const xod_network *net, int64_t n_atm, int64_t n_layers
  * kf, kr [n_reactions][ld], n, dist [n_species][ld] fp64, pred, via [n_species][ld] int32: device memory owned by the
  * caller; workspace >= xod_pathway_workspace_bytes (the edge weights, [2 n_reactions][columns]).
  * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, source out of range, tables unavailable: n_species or 2 n_reactions
- * >= 65535, or the tiles exceed shared memory), XOD_ERR_WORKSPACE, XOD_ERR_CUDA.
- * The equilibrium-chemistry start (NEXOCHEM / FASTCHEM) named beside it in SURVEY f4 is not built:
- * the paper gives no algorithm for it. */
+ * >= 65535, or the tiles exceed shared memory), XOD_ERR_WORKSPACE, XOD_ERR_CUDA. */
 size_t xod_pathway_workspace_bytes(const xod_network *net, int64_t ncol);
 xod_status xod_pathway(const xod_network *net, int64_t ncol, int64_t ld, const double *kf, const double *kr,
                        const double *n, int32_t source, double *dist, int32_t *pred, int32_t *via, void *workspace,
                        size_t workspace_bytes, void *stream);
+
+/* ---- f4: the thermochemical-equilibrium composition, the start the paper takes from its
+ * "built-in equilibrium chemistry solver" (the paper names the solver, not a method).
+ * Definition (reading E1): for every column the n >= 0 that minimises the Gibbs energy of an ideal gas
+ * mixture, G/RT = sum_i n_i (G_i/RT(T) + ln(n_i/N) + ln(P/P0)), N = sum_i n_i, P0 = 1 bar, among the compositions
+ * with sum_i a_ie n_i proportional to the element abundances b_e (a = the composition matrix given to
+ * xod_network_create, G_i/RT = the NASA-7 polynomial of xod_thermo), returned as number densities with
+ * sum_i n_i = P / (k_B T).  Equivalently (Lagrange conditions) G_i/RT + ln x_i + ln(P/P0) = sum_e a_ie pi_e for every
+ * species; at this composition every reversible reaction of the network has equal forward and reverse rates.
+ * Method: damped Newton iteration on the Lagrange conditions in (ln n_i, ln N) after Gordon & McBride, NASA RP-1311
+ * (1994), gas phase only; trace species are taken from the element potentials, so they are exact however small.
+ * b [n_elements][ld]: any positive scale, only ratios matter; an element whose composition column has entries of
+ * both signs (the charge) may have b = 0, i.e. a neutral gas; every other element needs b > 0.
+ * max_iter <= 0 selects 500, tol = 0 selects 1e-13 (largest abundance-weighted correction, and largest element residual relative to that
+ * element's own abundance, accepted).
+ * n [n_species][ld] out; pi [n_elements][ld] out, optional: the element potentials over RT; iters [ld] out, optional
+ * (int32): iterations used, NEGATIVE if max_iter was reached first, 0 if the column's inputs were rejected (T, P or b
+ * not positive and finite); in both failure cases the column of n and pi is NaN.  A numerically singular system (two
+ * elements that only ever occur together) shows up as non-convergence, not as an error.
+ * All arrays: device memory owned by the caller, column contiguous; no workspace (ln n_i is kept in n while the
+ * iteration runs).  Errors: XOD_ERR_INVALID_ARG (NULL, sizes, more than 16 elements, tol < 0), XOD_ERR_CUDA. */
+xod_status xod_equilibrium(const xod_network *net, int64_t ncol, int64_t ld, const double *T, const double *P,
+                           const double *b, int32_t max_iter, double tol, double *n, double *pi, int32_t *iters,
+                           void *stream);
 
 /* ---- end-to-end convenience: the fused call on HOST buffers (pinned for overlap; pageable works
  * but serialises).  Columns are processed in chunks of one round of tiles per SM through three

@@ -729,7 +729,9 @@ int orc_pathway(const orc_network *net, long ncol, long ld, const double *kf, co
  * lambda = min(1, 2 / max(5 |dlnN|, max over species with ln (n_i/N) > -18.42 of |dln n_i|),
  *              min over the other species with dln n_i > 0 of |(-ln (n_i/N) - 9.21) / (dln n_i - dlnN)|)
  * of the step.  Start: b scaled to sum 1, N = 0.1, n_i = 0.1 / n_species.  Converged when lambda = 1,
- * max_i n_i |dln n_i| / sum n <= tol, N |dlnN| / sum n <= tol and |sum_i a_ie n_i - b_e| <= tol max b for every e;
+ * max_i n_i |dln n_i| / sum n <= tol, N |dlnN| / sum n <= tol and |sum_i a_ie n_i - b_e| <= tol max(b_e,
+ * sum_i |a_ie| n_i) for every e (relative to the element's OWN abundance: a trace element carried by one inert
+ * species is decoupled from all the others, and only this residual sees it);
  * then ln n_i = ln N + sum_e a_ie pi_e - G_i/RT - ln (P / P0) is taken for EVERY species (trace species sit exactly
  * on the Lagrange condition).  The linear system is solved by Gaussian elimination with partial pivoting after each
  * row is divided by its largest entry (a charge row is many orders below the element rows).  Plain loops, one
@@ -762,7 +764,7 @@ int orc_equilibrium(const orc_network *net, long ncol, long ld, const double *T,
   int rc = 0;
   for (long col = 0; col < ncol && rc == 0; ++col) {
     const real_t Tc = (real_t)T[col], lnP = R_LOG((real_t)P[col] / P_REF);
-    real_t bsum = 0, bmax = 0;
+    real_t bsum = 0;
     for (int e = 0; e < ne; ++e) {
       b[e] = (real_t)b_in[(long)e * ld + col];
       int has_neg = 0;
@@ -771,10 +773,7 @@ int orc_equilibrium(const orc_network *net, long ncol, long ld, const double *T,
       if (b[e] > 0) bsum += b[e];
     }
     if (rc != 0) break;
-    for (int e = 0; e < ne; ++e) {
-      b[e] /= bsum;
-      if (R_FABS(b[e]) > bmax) bmax = R_FABS(b[e]);
-    }
+    for (int e = 0; e < ne; ++e) b[e] /= bsum;
     for (int i = 0; i < ns; ++i) {
       c[i] = nasa_g(nasa_set(net, i, Tc), Tc) + lnP;
       lnn[i] = R_LOG((real_t)0.1 / (real_t)ns);
@@ -828,13 +827,17 @@ int orc_equilibrium(const orc_network *net, long ncol, long ld, const double *T,
         if (w > err) err = w;
       }
       if (R_EXP(lnN) * R_FABS(dlnN) / newsum > err) err = R_EXP(lnN) * R_FABS(dlnN) / newsum;
-      real_t res = 0;
+      real_t res = 0;   /* per element, relative to its own abundance (to the charge carried, for a signed column) */
       for (int e = 0; e < ne; ++e) {
-        real_t s = -b[e];
-        for (int i = 0; i < ns; ++i) s += (real_t)net->composition[i * ne + e] * R_EXP(lnn[i]);
-        if (R_FABS(s) > res) res = R_FABS(s);
+        real_t s = -b[e], sa = 0;
+        for (int i = 0; i < ns; ++i) {
+          const real_t t = (real_t)net->composition[i * ne + e] * R_EXP(lnn[i]);
+          s += t, sa += R_FABS(t);
+        }
+        const real_t ref = b[e] > sa ? b[e] : sa;
+        if (R_FABS(s) > res * ref) res = R_FABS(s) / ref;
       }
-      done = lam == 1 && err <= (real_t)tol && res <= (real_t)tol * bmax;
+      done = lam == 1 && err <= (real_t)tol && res <= (real_t)tol;
     }
     if (rc != 0) break;
     const real_t ntot = (real_t)P[col] / (K_BOLTZ * Tc);

@@ -17,7 +17,7 @@ XOD_OK = 0
 XOD_UNI, XOD_BI, XOD_FALLOFF, XOD_PHOTO = 0, 1, 2, 3
 XOD_FLAG_SKIP_BALANCE_CHECK, XOD_FLAG_BUILD_LU = 1, 2
 XOD_TUNE_CHUNK_COLS, XOD_TUNE_TIMING, XOD_TUNE_SPLIT, XOD_TUNE_FUSED_KERNEL, XOD_TUNE_JAC_TILED = 0, 1, 2, 3, 4
-KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve", "photo_gemm", "photo_flux", "transport", "path_weights", "pathway"]
+KERNEL_NAMES = ["thermo", "prologue", "rates", "rates_from_k", "source", "jacobian", "fused", "fused_combine", "rate_coeffs", "jac_tiled", "newton_assemble", "lu_factor", "lu_solve", "photo_gemm", "photo_flux", "transport", "path_weights", "pathway", "equilibrium"]
 STATUS_NAMES = {0: "XOD_OK", 1: "XOD_ERR_INVALID_ARG", 2: "XOD_ERR_UNBALANCED", 3: "XOD_ERR_ALLOC",
                 4: "XOD_ERR_CUDA", 5: "XOD_ERR_WORKSPACE"}
 
@@ -30,7 +30,7 @@ EXPORTS = ["xod_network_create", "xod_network_destroy", "xod_last_error", "xod_n
            "xod_check_status", "xod_build_has_checks", "xod_network_jac_info", "xod_network_lu_info", "xod_network_lu_pattern",
            "xod_newton_workspace_bytes", "xod_newton_step", "xod_photo_create", "xod_photo_destroy",
            "xod_photo_workspace_bytes", "xod_photo_rates", "xod_transport",
-           "xod_pathway_workspace_bytes", "xod_pathway",
+           "xod_pathway_workspace_bytes", "xod_pathway", "xod_equilibrium",
            "xod_source_workspace_bytes_dndt", "xod_source_fused_workspace_bytes_dndt"]
 
 
@@ -273,6 +273,13 @@ class Network:
         _check(lib().xod_pathway(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(kf), _dp(kr), _dp(n), C.c_int32(source), _dp(dist),
                                  C.c_void_p(pred.data_ptr()), C.c_void_p(via.data_ptr()), _dp(workspace),
                                  C.c_size_t(0 if workspace is None else workspace.numel() * 8), _stream(stream)))
+
+    # ---- f4: thermochemical-equilibrium composition (n, pi fp64, iters int32 tensors)
+    def equilibrium(self, ncol, ld, T, P, b, n, pi=None, iters=None, max_iter=0, tol=0.0, stream=None):
+        assert iters is None or (iters.is_cuda and iters.element_size() == 4)
+        _check(lib().xod_equilibrium(self._h, C.c_int64(ncol), C.c_int64(ld), _dp(T), _dp(P), _dp(b), C.c_int32(max_iter),
+                                     C.c_double(tol), _dp(n), _dp(pi), None if iters is None else C.c_void_p(iters.data_ptr()),
+                                     _stream(stream)))
 
     # ---- end to end on HOST buffers (numpy arrays or pinned torch CPU tensors)
     def source_fused_host(self, ncol, ld, T, P, J, n, dndt):

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 CHECKED = bool(os.environ.get("XOD_CHECK"))   # debugging build: bounds-checked table indices (csrc/xod_cta.cuh)
 LIB = os.path.join(HERE, "libxodiac_check.so" if CHECKED else "libxodiac.so")
 SOURCES = ["api.cu", "pack.cpp", "pack_fused.cpp", "pack_jac.cpp", "pack_lu.cpp", "pack_path.cpp"]
-HEADERS = ["kernels.cuh", "fused.cuh", "jac_tiled.cuh", "newton.cuh", "photo.cuh", "transport.cuh", "pathway.cuh", "sched.cuh", "rates2.cuh", "xod_math.cuh", "xod_cta.cuh", "xod_internal.h", os.path.join("..", "..", "include", "xodiac.h")]
+HEADERS = ["kernels.cuh", "fused.cuh", "jac_tiled.cuh", "newton.cuh", "photo.cuh", "transport.cuh", "pathway.cuh", "equil.cuh", "sched.cuh", "rates2.cuh", "xod_math.cuh", "xod_cta.cuh", "xod_internal.h", os.path.join("..", "..", "include", "xodiac.h")]
 
 
 def _stale():

@@ -13,6 +13,7 @@
 #include "photo.cuh"
 #include "transport.cuh"
 #include "pathway.cuh"
+#include "equil.cuh"
 #include "rates2.cuh"
 #include "kernels.cuh"
 
@@ -279,6 +280,18 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (st == XOD_OK) {
         cudaError_t ce = cudaFuncSetAttribute(k_pathway, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
         if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_pathway)");
+      }
+    }
+    if (h.ne > 0 && h.ne <= kEqMaxElem) {   // f4: composition lists of xod_equilibrium
+      EquilDev &ed = net->ed;
+      ed.ns = h.ns, ed.ne = h.ne;
+      if (st == XOD_OK) st = upload(net, h.eq_ptr, &ed.sp_ptr);
+      if (st == XOD_OK) st = upload(net, h.eq_ea, &ed.sp_ea);
+      if (st == XOD_OK) st = upload(net, h.eq_neg, &ed.el_neg);
+      ed.nasa = d.nasa, ed.tmid = d.tmid;
+      if (st == XOD_OK) {
+        cudaError_t ce = cudaFuncSetAttribute(k_equilibrium, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
+        if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_equilibrium)");
       }
     }
     if (h.lu.enabled) {
@@ -1108,6 +1121,33 @@ xod_status xod_pathway(const xod_network *net, int64_t ncol, int64_t ld, const d
     k_pathway<<<grid, kFWarps * 32, path_smem_bytes(net->h.ns), s>>>(net->pd, a);
     XOD_CUDA(cudaGetLastError());
   }
+  return XOD_OK;
+}
+
+// ---------------------------------------------------------------------------- f4: equilibrium composition
+
+xod_status xod_equilibrium(const xod_network *net, int64_t ncol, int64_t ld, const double *T, const double *P,
+                           const double *b, int32_t max_iter, double tol, double *n, double *pi, int32_t *iters,
+                           void *stream) {
+  xod_status st = check_common(net, ncol, ld);
+  if (st != XOD_OK) return st;
+  if (net->h.ne <= 0 || net->h.ne > kEqMaxElem)
+    return fail(XOD_ERR_INVALID_ARG, "xod_equilibrium supports 1 to 16 elements (including a charge column)");
+  if (net->h.ns <= 0) return fail(XOD_ERR_INVALID_ARG, "the network has no species");
+  if (ncol == 0) return XOD_OK;
+  if (!T || !P || !b || !n) return fail(XOD_ERR_INVALID_ARG, "T, P, b or n is NULL");
+  if (tol < 0 || tol != tol) return fail(XOD_ERR_INVALID_ARG, "tol must be >= 0 (0 selects the default 1e-13)");
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  EquilArgs a{};
+  a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.b = b, a.n = n, a.pi = pi, a.iters = iters;
+  a.max_iter = max_iter > 0 ? max_iter : 500;
+  a.tol = tol > 0 ? tol : 1.0e-13;
+  const size_t smem = (size_t)equil_smem_doubles(net->h.ne) * kEqThreads * sizeof(double);
+  {
+    Timed tm(net, KID_EQUILIBRIUM, s);
+    k_equilibrium<<<(unsigned)((ncol + kEqThreads - 1) / kEqThreads), kEqThreads, smem, s>>>(net->ed, a);
+  }
+  XOD_CUDA(cudaGetLastError());
   return XOD_OK;
 }
 

@@ -91,6 +91,16 @@ xod_status pack_network(const xod_network_desc *d, HostTables &h, std::string &e
     if (!std::isfinite(d->t_mid[i])) return err = fmt("species %ld: t_mid not finite", i), XOD_ERR_INVALID_ARG;
 
   h.ns = ns, h.ne = ne, h.nr = nr;
+  // composition as short (element, count) lists per species (xod_equilibrium); which columns carry both signs
+  h.eq_ptr.assign(1, 0), h.eq_ea.clear(), h.eq_neg.assign((size_t)ne, 0);
+  for (int i = 0; i < ns; ++i) {
+    for (int e = 0; e < ne; ++e) {
+      const int32_t a = d->composition[(size_t)i * ne + e];
+      if (a < 0) h.eq_neg[e] = 1;
+      if (a != 0 && e < 256) h.eq_ea.push_back(a * 256 + e);
+    }
+    h.eq_ptr.push_back((int32_t)h.eq_ea.size());
+  }
   h.uni_begin = 0;
   h.bi_begin = counts[XOD_UNI];
   h.fo_begin = h.bi_begin + counts[XOD_BI];

@@ -186,8 +186,20 @@ struct PathDev {
   const PathTask *sched;
 };
 
+// ---- tables of the equilibrium-composition kernel (f4: xod_equilibrium; equil.cuh) ----------------
+constexpr int kEqThreads = 64;      // columns per CTA
+constexpr int kEqMaxElem = 16;      // elements (including a charge column) the shared-memory layout is sized for
+struct EquilDev {
+  int32_t ns, ne;
+  const int32_t *sp_ptr;    // [ns + 1] into sp_ea
+  const int32_t *sp_ea;     // element + 256 * count (count signed: a charge column has both signs)
+  const int32_t *el_neg;    // [ne] 1 if the element's composition column has a negative entry (abundance 0 allowed)
+  const double *nasa, *tmid;
+};
+
 struct HostTables {
   int32_t ns = 0, ne = 0, nr = 0, n_photo = 0;
+  std::vector<int32_t> eq_ptr, eq_ea, eq_neg;   // composition as (element, count) lists per species; signed columns
   int32_t uni_begin = 0, bi_begin = 0, fo_begin = 0, ph_begin = 0;
   std::vector<int32_t> packed_to_user, user_to_packed, photo_user;
   std::vector<double> c0, c1, c2, l0, l1, l2, fcl, cN;
@@ -238,7 +250,7 @@ size_t jac_tiled_smem_bytes(int ns, int acc_rows, int chunk, int meta_cap);
 // optional per-kernel timing (xod_network_tune(XOD_TUNE_TIMING)): CUDA event pairs recorded around
 // every launch on the caller's stream, summed by xod_network_timing_read
 namespace xod {
-enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_TRANSPORT, KID_PATH_WEIGHTS, KID_PATHWAY, KID_COUNT };
+enum KernelId { KID_THERMO = 0, KID_PROLOGUE, KID_RATES, KID_RATES_FROM_K, KID_SOURCE, KID_JACOBIAN, KID_FUSED, KID_FUSED_COMBINE, KID_RATE_COEFFS, KID_JAC_TILED, KID_NEWTON_ASSEMBLE, KID_LU_FACTOR, KID_LU_SOLVE, KID_PHOTO_GEMM, KID_PHOTO_FLUX, KID_TRANSPORT, KID_PATH_WEIGHTS, KID_PATHWAY, KID_EQUILIBRIUM, KID_COUNT };
 struct TimingState {
   bool on = false;
   std::vector<void *> pool;                       // cudaEvent_t, reused
@@ -267,6 +279,7 @@ struct xod_network {
   xod::JacTiledDev jd{};
   xod::LuDev ld{};
   xod::PathDev pd{};
+  xod::EquilDev ed{};
   int64_t force_split = 0;  // XOD_TUNE_SPLIT: 0 = automatic
   int64_t use_fused = 1;    // XOD_TUNE_FUSED_KERNEL: 0 = always the multi-kernel path
   int64_t use_jac_tiled = 1;  // XOD_TUNE_JAC_TILED: 0 = the one-warp-per-entry gather kernel

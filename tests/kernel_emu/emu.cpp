@@ -33,6 +33,7 @@ int emu_syncthreads_or(int predicate) {   // barrier with an OR reduction over t
 #include "../../paper_2512_06729_b200/csrc/photo.cuh"
 #include "../../paper_2512_06729_b200/csrc/transport.cuh"
 #include "../../paper_2512_06729_b200/csrc/pathway.cuh"
+#include "../../paper_2512_06729_b200/csrc/equil.cuh"
 #include "../../paper_2512_06729_b200/csrc/kernels.cuh"
 
 namespace xod {
@@ -332,6 +333,23 @@ int emu_pathway(const xod_network_desc *desc, int64_t ncol, int64_t ld, const do
   a.ntiles = (int32_t)((ncol + kFW - 1) / kFW);
   run_grid((unsigned)((ncol + 127) / 128), 3, 128, false, [&] { k_path_weights(d, a, (h.nr + 2) / 3); });
   run_grid((unsigned)grid, 1, kFWarps * 32, true, [&] { k_pathway(pd, a); });
+  return 0;
+}
+
+// f4: equilibrium composition: k_equilibrium (thread = column, no barrier: threads run one after another)
+int emu_equilibrium(const xod_network_desc *desc, int64_t ncol, int64_t ld, const double *T, const double *P, const double *b,
+                    int max_iter, double tol, double *n, double *pi, int32_t *iters) {
+  HostTables h;
+  std::string err;
+  if (pack_network(desc, h, err) != XOD_OK || ncol <= 0 || h.ne <= 0 || h.ne > kEqMaxElem) return 1;
+  if ((size_t)equil_smem_doubles(h.ne) * kEqThreads * sizeof(double) > sizeof(smem_raw)) return 2;
+  EquilDev d{};
+  d.ns = h.ns, d.ne = h.ne, d.sp_ptr = h.eq_ptr.data(), d.sp_ea = h.eq_ea.data(), d.el_neg = h.eq_neg.data();
+  d.nasa = h.nasa.data(), d.tmid = h.tmid.data();
+  EquilArgs a{};
+  a.ncol = ncol, a.ld = ld, a.T = T, a.P = P, a.b = b, a.n = n, a.pi = pi, a.iters = iters;
+  a.max_iter = max_iter > 0 ? max_iter : 500, a.tol = tol > 0 ? tol : 1e-13;
+  run_grid((unsigned)((ncol + kEqThreads - 1) / kEqThreads), 1, kEqThreads, false, [&] { k_equilibrium(d, a); });
   return 0;
 }
 

@@ -55,4 +55,4 @@ inline long min(long a, long b) { return a < b ? a : b; }
 inline long max(long a, long b) { return a > b ? a : b; }
 inline long long min(long long a, long long b) { return a < b ? a : b; }
 inline long long max(long long a, long long b) { return a > b ? a : b; }
-using std::fabs; using std::fma; using std::fmax; using std::fmin; using std::log; using std::log2;
+using std::exp; using std::fabs; using std::fma; using std::fmax; using std::fmin; using std::log; using std::log2;

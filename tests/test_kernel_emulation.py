@@ -19,7 +19,7 @@ EMU_DIR = os.path.join(ROOT, "tests", "kernel_emu")
 CSRC = os.path.join(ROOT, "paper_2512_06729_b200", "csrc")
 LIB = os.path.join(EMU_DIR, "libxod_emu.so")
 SOURCES = [os.path.join(EMU_DIR, "emu.cpp")] + [os.path.join(CSRC, f) for f in ("pack.cpp", "pack_fused.cpp", "pack_jac.cpp", "pack_lu.cpp", "pack_path.cpp")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "jac_tiled.cuh", "newton.cuh", "photo.cuh", "transport.cuh", "pathway.cuh", "sched.cuh", "xod_math.cuh", "xod_internal.h")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("fused.cuh", "rates2.cuh", "kernels.cuh", "jac_tiled.cuh", "newton.cuh", "photo.cuh", "transport.cuh", "pathway.cuh", "equil.cuh", "sched.cuh", "xod_math.cuh", "xod_internal.h")] + [
     os.path.join(EMU_DIR, "shim", "cuda_runtime.h"), os.path.join(EMU_DIR, "shim", "xod_cta.cuh")]
 
 
