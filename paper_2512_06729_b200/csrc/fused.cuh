@@ -128,7 +128,13 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       const int c = tid & (kFW - 1);
       const int64_t gc = min(col0 + c, a.ncol - 1);
       // all loads of the tile in flight at once (cp.async), not one round trip per row
-      for (int i = tid >> 4; i < ns; i += (kFWarps * 32) >> 4) cp_async8(n_s + i * kFW + c, a.n + (size_t)i * a.ld + gc);
+      if (col0 + kFW <= a.ncol && ((reinterpret_cast<uintptr_t>(a.n) | ((size_t)a.ld * sizeof(double))) & 15) == 0) {
+        // a full tile whose rows are 16-byte aligned: two columns per copy
+        for (int u = tid; u < ns * (kFW / 2); u += kFWarps * 32)
+          cp_async16(n_s + u * 2, a.n + (size_t)(u >> 3) * a.ld + col0 + (u & 7) * 2);
+      } else {
+        for (int i = tid >> 4; i < ns; i += (kFWarps * 32) >> 4) cp_async8(n_s + i * kFW + c, a.n + (size_t)i * a.ld + gc);
+      }
       for (int i = tid; i < f.n_acc * kFW; i += kFWarps * 32) acc_s[i] = 0.0;
       if (tid < kFW) {
         n_s[ns * kFW + tid] = 1.0;
