@@ -284,6 +284,10 @@ def stage_timings(binding, h3, net, dev, ws_for, dfma_per_s):
         if big:
             jac = torch.empty((h3.nnz_jac, ld), dtype=torch.float64, device="cuda")
             calls["jacobian"] = lambda: h3.jacobian(ncol, ld, kf, kr, n, jac)
+            # the production / loss variants (P_y and L_y of Eq. 1 separately) run the multi-kernel pipeline
+            pr, lo = torch.empty_like(d), torch.empty_like(d)
+            calls["source_fused_prod_loss"] = lambda: h3.source_fused(ncol, ld, T, P, J, n, d, pr, lo, workspace=ws)
+            calls["source_prod_loss"] = lambda: h3.source(ncol, ld, kf, kr, n, d, pr, lo, workspace=ws)
 
             def jac_gather():
                 h3.tune(binding.XOD_TUNE_JAC_TILED, 0)
