@@ -605,3 +605,55 @@ def test_production_and_loss_over_several_column_chunks(xod, oracle, network):
             assert np.all(np.isnan(G.host(d0)[:, ncol:])) and np.all(np.isnan(G.host(p0)[:, ncol:]))
         h.check_status()
         h.close()
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14, 15, 16])
+def test_random_networks(xod, oracle, seed):
+    """The seeded random networks of tests/test_kernel_emulation.py (odd segment lengths, reaction counts around
+    the chunk size, irreversible reactions and Kooij forms mixed in, ragged column counts, cold and hot columns)
+    through xod_rate_coeffs, xod_source_fused, xod_source and xod_jacobian, reaction-split or not."""
+    from paper_2512_06729_b200 import synth
+    rng = np.random.default_rng(seed)
+    elements = ["H", "C", "O", "N", "S"][:int(rng.integers(2, 6))]
+    ns = int(rng.integers(6, 40))
+    nr = int(rng.integers(5, 330))
+    net = synth.make_network(900 + seed, elements, ns, nr, inert=())
+    flip = rng.random(net.n_reactions) < 0.3
+    net.reversible = np.where(flip & (net.type != 3), 0, net.reversible).astype(np.uint8)
+    net.t_ref = np.where(rng.random(net.n_reactions) < 0.3, 300.0, 1.0)
+    n_layers = int(rng.integers(3, 45))
+    atm = synth.make_atmosphere(1900 + seed, net, 1, n_layers, t_shift=(-300.0, 300.0))
+    ncol, ld = atm.ncol, atm.ld
+    h = xod.Network(net, device=0)
+    h.selfcheck()
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    dT, dP, dJ, dn = (G.dev(a) for a in (atm.T, atm.P, atm.J, atm.n))
+    ws = G.workspace(max(h.source_fused_workspace_bytes(ncol), h.source_workspace_bytes(ncol), h.rate_coeffs_workspace_bytes(ncol)) + (8 << 20))
+    kf, kr = G.empty(net.n_reactions, ld), G.empty(net.n_reactions, ld)
+    h.rate_coeffs(ncol, ld, dT, dP, dJ, kf, kr, ws)
+    G.check_k(G.host(kf)[:, :ncol], okf[:, :ncol], "random net %d k_f" % seed)
+    G.check_k(G.host(kr)[:, :ncol], okr[:, :ncol], "random net %d k_r" % seed)
+    assert np.all(G.host(kr)[net.reversible == 0, :ncol] == 0.0)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    okr_f = np.where(np.isfinite(okr), okr, 0.0)
+    want_f, wpf, wlf = oracle.source(net, okf, okr_f, atm.n, ncol)
+    dkf, dkr = G.dev(okf), G.dev(okr_f)
+    for split in (0, 2):
+        h.tune(xod.XOD_TUNE_SPLIT, split)
+        d0 = G.empty(ns, ld)
+        h.source_fused(ncol, ld, dT, dP, dJ, dn, d0, workspace=ws)
+        G.check_sum_entries(G.host(d0), want, wp + wl, ncol, "random net %d xod_source_fused split %d" % (seed, split))
+        d1 = G.empty(ns, ld)
+        h.source(ncol, ld, dkf, dkr, dn, d1, workspace=ws)
+        G.check_sum_entries(G.host(d1), want_f, wpf + wlf, ncol, "random net %d xod_source split %d" % (seed, split))
+        assert np.all(np.isnan(G.host(d0)[:, ncol:])) and np.all(np.isnan(G.host(d1)[:, ncol:]))
+    h.tune(xod.XOD_TUNE_SPLIT, 0)
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr_f, atm.n, rp, col, ncol)
+    for tiled in (1, 0):
+        h.tune(xod.XOD_TUNE_JAC_TILED, tiled)
+        jac = G.empty(h.nnz_jac, ld)
+        h.jacobian(ncol, ld, dkf, dkr, dn, jac)
+        G.check_sum_entries(G.host(jac), wj, sj, ncol, "random net %d xod_jacobian (tiled %d)" % (seed, tiled))
+    h.check_status()
+    h.close()

@@ -458,3 +458,54 @@ def test_barrier_synchronised_kernel_sources_are_race_free_under_thread_sanitize
                          timeout=900)
     assert "emulated-ok" in out.stdout, out.stderr[-2000:]
     assert "ThreadSanitizer" not in out.stderr, out.stderr[-3000:]
+
+
+@pytest.mark.parametrize("seed", [11, 12, 13, 14, 15, 16])
+def test_random_networks_through_the_kernel_sources(emu, oracle, seed):
+    """Seeded random networks of odd sizes (segment lengths that are not multiples of 4, reaction counts around
+    the chunk size, one to five elements, some reactions made irreversible, Kooij forms mixed in) and ragged column
+    counts through k_fused (both modes, split or not), k_rate_coeffs and k_jac_tiled against the oracle: the
+    packer's padding, chunking and schedules must hold for shapes nobody picked by hand; xod_network_selfcheck
+    must accept the tables."""
+    from paper_2512_06729_b200 import synth
+    rng = np.random.default_rng(seed)
+    elements = ["H", "C", "O", "N", "S"][:int(rng.integers(2, 6))]
+    ns = int(rng.integers(6, 40))
+    nr = int(rng.integers(5, 330))
+    net = synth.make_network(900 + seed, elements, ns, nr, inert=())
+    flip = rng.random(net.n_reactions) < 0.3
+    net.reversible = np.where(flip & (net.type != 3), 0, net.reversible).astype(np.uint8)
+    net.t_ref = np.where(rng.random(net.n_reactions) < 0.3, 300.0, 1.0)
+    n_layers = int(rng.integers(3, 45))
+    atm = synth.make_atmosphere(1900 + seed, net, 1, n_layers, t_shift=(-300.0, 300.0))
+    ncol, ld = atm.ncol, atm.ld
+    h = binding.Network(net, device=-1)
+    h.selfcheck()
+    d, keep = descriptor(net)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    # rate coefficients (reading R5 rules)
+    kf, kr = np.full((net.n_reactions, ld), np.nan), np.full((net.n_reactions, ld), np.nan)
+    assert emu.emu_rate_coeffs(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J), ptr(kf), ptr(kr),
+                               C.c_int(8)) == 0
+    G.check_k(kf[:, :ncol], okf[:, :ncol], "random net %d k_f" % seed)
+    G.check_k(kr[:, :ncol], okr[:, :ncol], "random net %d k_r" % seed)
+    assert np.all(kr[net.reversible == 0, :ncol] == 0.0)
+    # source term, evaluated and from stored coefficients, split or not
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    scale = wp + wl
+    okr_f = np.where(np.isfinite(okr), okr, 0.0)
+    want_f, wpf, wlf = oracle.source(net, okf, okr_f, atm.n, ncol)
+    for nsplit in (1, 2):
+        got = run_fused(emu, net, atm, ncol, grid=2, nsplit=nsplit)
+        G.check_sum_entries(got, want, scale, ncol, "random net %d k_fused split %d" % (seed, nsplit))
+        got = run_fused(emu, net, atm, ncol, kf=okf, kr=okr_f, grid=3, nsplit=nsplit)
+        G.check_sum_entries(got, want_f, wpf + wlf, ncol, "random net %d k_fused<FROMK> split %d" % (seed, nsplit))
+    # Jacobian values
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr_f, atm.n, rp, col, ncol)
+    jac = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr_f), ptr(atm.n), ptr(jac),
+                                  C.c_int(2), C.c_int(2)) == 0
+    G.check_sum_entries(jac, wj, sj, ncol, "random net %d k_jac_tiled" % seed)
+    print("random network %d: %d species, %d reactions (%d irreversible), %d columns: ok" % (
+        seed, net.n_species, net.n_reactions, int((net.reversible == 0).sum()), ncol))
