@@ -223,8 +223,9 @@ xod_status xod_jacobian(const xod_network *net, int64_t ncol, int64_t ld, const 
  * A zero pivot gives IEEE inf/NaN in that column (no pivoting, no error).
  * Errors: XOD_ERR_INVALID_ARG (NULL, sizes, network created without XOD_FLAG_BUILD_LU or without the
  * single-kernel tables), XOD_ERR_WORKSPACE, XOD_ERR_CUDA.
- * xod_network_lu_info: info[5] = enabled, nonzeros of L + U (with fill), (row, pivot) pairs, multiply-add
- * updates of one factorisation, longest row.  xod_network_lu_pattern: perm[p] = species eliminated p-th;
+ * xod_network_lu_info: info[8] = enabled, nonzeros of L + U (with fill), (row, pivot) pairs, multiply-add
+ * updates of one factorisation, longest row, rows factorised together per block, U values read per column by the
+ * block schedule (its memory traffic / 8 bytes; without blocks it would equal the updates), pivot steps.  xod_network_lu_pattern: perm[p] = species eliminated p-th;
  * row p of the filled pattern = permuted column indices, ascending (L part, diagonal, U part). */
 xod_status xod_network_lu_info(const xod_network *net, int64_t *info);
 xod_status xod_network_lu_pattern(const xod_network *net, int32_t *perm, int64_t *row_ptr, int32_t *col);

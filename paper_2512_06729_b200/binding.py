@@ -171,9 +171,9 @@ class Network:
         return dict(zip(keys, [int(x) for x in v]))
 
     def lu_info(self):
-        v = (C.c_int64 * 5)()
+        v = (C.c_int64 * 8)()
         _check(lib().xod_network_lu_info(self._h, v))
-        return dict(zip(("enabled", "nnz_lu", "pairs", "updates", "max_row"), [int(x) for x in v]))
+        return dict(zip(("enabled", "nnz_lu", "pairs", "updates", "max_row", "block_rows", "u_loads", "steps"), [int(x) for x in v]))
 
     def lu_pattern(self):
         info = self.lu_info()

@@ -306,6 +306,10 @@ xod_status xod_network_create(const xod_network_desc *desc, int cuda_device, xod
       if (st == XOD_OK) st = upload(net, u.rows, &ud.rows);
       if (st == XOD_OK) st = upload(net, u.pairs, &ud.pairs);
       if (st == XOD_OK) st = upload(net, u.tgt, &ud.tgt);
+      ud.block_rows = u.block_rows, ud.n_blocks = (int32_t)u.blocks.size();
+      if (st == XOD_OK) st = upload(net, u.blocks, &ud.blocks);
+      if (st == XOD_OK) st = upload(net, u.steps, &ud.steps);
+      if (st == XOD_OK) st = upload(net, u.items, &ud.items);
       if (st == XOD_OK) {
         cudaError_t ce = cudaFuncSetAttribute(k_lu_factor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFusedSmemMax);
         if (ce != cudaSuccess) st = cuda_fail(ce, "cudaFuncSetAttribute(k_lu_factor)");
@@ -853,6 +857,7 @@ xod_status xod_network_lu_info(const xod_network *net, int64_t *info) {
   if (!net || !info) return fail(XOD_ERR_INVALID_ARG, "NULL argument");
   const LuHost &u = net->h.lu;
   info[0] = u.enabled, info[1] = u.nnz, info[2] = (int64_t)u.pairs.size(), info[3] = u.n_updates, info[4] = u.max_row;
+  info[5] = u.block_rows, info[6] = u.n_block_loads, info[7] = (int64_t)u.steps.size();
   return XOD_OK;
 }
 
@@ -869,7 +874,7 @@ xod_status xod_network_lu_pattern(const xod_network *net, int32_t *perm, int64_t
 }  // extern "C"
 
 namespace {
-constexpr int64_t kNewtonChunk = 2048;   // columns per pass of the implicit step (bounds the workspace)
+constexpr int64_t kNewtonChunk = 2368;   // columns per pass of the implicit step (bounds the workspace): 148 SMs x 16 = two full waves of k_lu_factor's 8-column CTAs
 int64_t newton_chunk(int64_t ncol) { return std::min<int64_t>(round_up(std::max<int64_t>(ncol, 1), 32), kNewtonChunk); }
 }  // namespace
 
@@ -903,7 +908,7 @@ xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, con
   double *f = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(workspace) + 255) & ~uintptr_t(255));
   double *rhs = f + ns * cw, *jac = rhs + ns * cw, *lu = jac + nnzj * cw;
   void *src_ws = lu + nnzl * cw;
-  const size_t smem = (size_t)net->h.lu.max_row * 32 * sizeof(double);
+  const size_t smem = (size_t)net->h.lu.block_rows * net->h.lu.max_row * kLuCols * sizeof(double);
   if (smem > kFusedSmemMax) return fail(XOD_ERR_INVALID_ARG, "a row of the LU pattern does not fit shared memory");
   for (int64_t c0 = 0; c0 < ncol; c0 += cw) {
     const int64_t w = std::min(cw, ncol - c0);
@@ -923,7 +928,7 @@ xod_status xod_newton_step(const xod_network *net, int64_t ncol, int64_t ld, con
     }
     {
       Timed tm(net, KID_LU_FACTOR, s);
-      k_lu_factor<<<(unsigned)((w + 31) / 32), 32 * kLuWarps, smem, s>>>(net->ld, lu, cw, w);
+      k_lu_factor<<<(unsigned)((w + kLuCols - 1) / kLuCols), 32 * kLuWarps, smem, s>>>(net->ld, lu, cw, w);
       XOD_CUDA(cudaGetLastError());
     }
     {

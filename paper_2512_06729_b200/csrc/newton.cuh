@@ -6,9 +6,10 @@
 // order n_species per column, all with the SAME pattern (pack_lu.cpp: minimum-degree order, filled
 // pattern, update schedule), lanes = columns, values in [position][column] arrays:
 //   k_newton_assemble  A = I - dt Jac scattered into the filled LU storage (fill = 0); rhs = -F permuted
-//   k_lu_factor        row-by-row LU without pivoting (the order is fixed by the pattern, as in DLSODES'
-//                      sparse solver); CTA = 32 columns x kLuWarps warps; row i sits in shared memory
-//                      while the warps share the updates a_ij -= l_ik a_kj of each pivot k in L(i)
+//   k_lu_factor        LU without pivoting (the order is fixed by the pattern, as in DLSODES' sparse solver), blocks
+//                      of rows at a time: CTA = 8 columns x 64 entry slices; the rows of a block sit in shared
+//                      memory while the updates a_ij -= l_ik a_kj of each pivot k are shared by the threads and
+//                      the pivot's U row is read once per block
 //   k_lu_solve         forward / backward substitution, delta scattered back to species order, y += delta
 // Atomic-free and deterministic.  Division by a zero pivot gives IEEE inf/NaN, not an error.
 #pragma once
@@ -50,42 +51,83 @@ __global__ void __launch_bounds__(128) k_newton_assemble(LuDev u, NewtonArgs a) 
   }
 }
 
-// grid ceil(ncol / 32); block 32 x kLuWarps; dynamic shared memory max_row x 32 doubles
+// grid ceil(ncol / kLuCols); block 32 x kLuWarps = 64 entry slices x kLuCols columns; dynamic shared memory
+// block_rows x max_row x kLuCols doubles.  Blocks of consecutive rows (pack_lu.cpp) are factorised together: the
+// rows sit in shared memory as [slot][column] while the pivots of the union of their L parts are applied in
+// ascending order, one barrier per pivot; the pivot's U row is read once (global memory, or the block's own rows
+// when the pivot lies inside the block) and applied to every row of the block that holds a_ik.  On write-back the
+// L part is stored as l_ik = a_ik / a_kk and the DIAGONAL AS ITS RECIPROCAL (so that neither later blocks nor
+// k_lu_solve divide).  Idle column lanes of a ragged last CTA only take part in the barriers.
 __global__ void __launch_bounds__(32 * kLuWarps) k_lu_factor(LuDev u, double *lu, int64_t ldw, int64_t ncol) {
   double *w = reinterpret_cast<double *>(cta_dyn_smem());
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int64_t c = (int64_t)blockIdx.x * 32 + lane;
-  const bool valid = c < ncol;   // idle lanes of a ragged group only take part in the barriers
-  double *col = lu + (valid ? c : 0);
-  for (int i = 0; i < u.n; ++i) {
-    const LuRow row = u.rows[i];
+  const int c = threadIdx.x & (kLuCols - 1), es = threadIdx.x / kLuCols;
+  constexpr int kSlices = 32 * kLuWarps / kLuCols;
+  const int64_t gc = (int64_t)blockIdx.x * kLuCols + c;
+  const bool valid = gc < ncol;
+  double *col = lu + (valid ? gc : 0);
+  double *wc = w + c;
+  const int wslots = u.block_rows * u.max_row;
+  (void)wslots;
+  for (int bi = 0; bi < u.n_blocks; ++bi) {
+    const LuBlock blk = u.blocks[bi];
     if (valid)
-      for (int t = warp; t < row.len; t += kLuWarps)
-        w[XOD_IDX(t, u.max_row) * 32 + lane] = col[(size_t)XOD_IDX((int64_t)row.begin + t, u.nnz) * ldw];
+      for (int b = 0; b < blk.nrows; ++b) {
+        const LuRow row = u.rows[XOD_IDX(blk.row0 + b, u.n)];
+        for (int t = es; t < row.len; t += kSlices)
+          wc[(size_t)XOD_IDX(b * u.max_row + t, wslots) * kLuCols] = col[(size_t)XOD_IDX((int64_t)row.begin + t, u.nnz) * ldw];
+      }
     __syncthreads();
-    for (int pi = row.pair_begin; pi < row.pair_end; ++pi) {
-      const LuPair pr = u.pairs[pi];
+    for (int si = blk.step_begin; si < blk.step_end; ++si) {
+      const LuStep st = u.steps[si];
       if (valid) {
-        // a_ik is final here: pivots k' < k have been applied (barrier below), pivots >= k never touch it
-        const double l = w[XOD_IDX(pr.t_k, row.len) * 32 + lane] / col[(size_t)XOD_IDX((int64_t)pr.diag_k, u.nnz) * ldw];
-        const double *urow = col + (size_t)(pr.diag_k + 1) * ldw;
-        const uint16_t *tg = u.tgt + pr.tgt_off;
-        for (int jj = warp; jj < pr.cnt; jj += kLuWarps) {
-          (void)XOD_IDX((int64_t)pr.diag_k + 1 + jj, u.nnz);
-          double *dst = w + XOD_IDX((int)tg[jj], row.len) * 32 + lane;
-          *dst = fma(-l, urow[(size_t)jj * ldw], *dst);
+        // a_ik of every item is final here: pivots below k have been applied (barrier), pivots >= k never touch it
+        const double rd = st.src >= 0 ? 1.0 / wc[(size_t)XOD_IDX(st.src - 1, wslots) * kLuCols]
+                                      : col[(size_t)XOD_IDX((int64_t)st.diag_k, u.nnz) * ldw];
+        double l[kLuMaxBlockRows];
+        int base[kLuMaxBlockRows];
+        const uint16_t *tg[kLuMaxBlockRows];
+#pragma unroll
+        for (int x = 0; x < kLuMaxBlockRows; ++x) {
+          l[x] = 0.0, base[x] = 0, tg[x] = u.tgt;
+          if (x < st.n_items) {
+            const LuItem item = u.items[st.item_begin + x];
+            l[x] = wc[(size_t)XOD_IDX(item.slot_ik, wslots) * kLuCols] * rd;
+            base[x] = item.base, tg[x] = u.tgt + item.tgt_off;
+          }
+        }
+        const double *urow = col + (size_t)(st.diag_k + 1) * ldw;
+        for (int jj = es; jj < st.cnt; jj += kSlices) {
+          (void)XOD_IDX((int64_t)st.diag_k + 1 + jj, u.nnz);
+          const double uv = st.src >= 0 ? wc[(size_t)XOD_IDX(st.src + jj, wslots) * kLuCols] : urow[(size_t)jj * ldw];
+#pragma unroll
+          for (int x = 0; x < kLuMaxBlockRows; ++x)
+            if (x < st.n_items) {
+              double *dst = wc + (size_t)XOD_IDX(base[x] + (int)tg[x][jj], wslots) * kLuCols;
+              *dst = fma(-l[x], uv, *dst);
+            }
         }
       }
       __syncthreads();
     }
-    const int n_l = row.pair_end - row.pair_begin;   // the L part: store l_ik = a_ik / a_kk
     if (valid)
-      for (int t = warp; t < row.len; t += kLuWarps) {
-        double v = w[t * 32 + lane];
-        if (t < n_l) v /= col[(size_t)u.pairs[row.pair_begin + t].diag_k * ldw];
-        col[(size_t)(row.begin + t) * ldw] = v;
+      for (int b = 0; b < blk.nrows; ++b) {
+        const int i = blk.row0 + b;
+        const LuRow row = u.rows[i];
+        const int n_l = row.pair_end - row.pair_begin;
+        for (int t = es; t < row.len; t += kSlices) {
+          double v = wc[(size_t)(b * u.max_row + t) * kLuCols];
+          if (t < n_l) {        // L part: l_ik = a_ik / a_kk; the pivot row is an earlier block's (reciprocal stored) or this block's
+            const int k = XOD_IDX(__ldg(u.col + row.begin + t), u.n);
+            const int dslot = __ldg(u.diag + k) - (int)__ldg(u.row_ptr + k);
+            v *= k >= blk.row0 ? 1.0 / wc[(size_t)XOD_IDX((k - blk.row0) * u.max_row + dslot, wslots) * kLuCols]
+                               : col[(size_t)__ldg(u.diag + k) * ldw];
+          } else if (t == n_l) {
+            v = 1.0 / v;        // the diagonal is stored as its reciprocal
+          }
+          col[(size_t)(row.begin + t) * ldw] = v;
+        }
       }
-    __syncthreads();   // row i is in global memory before later rows read it; w may be overwritten
+    __syncthreads();   // the block is in global memory before later blocks read it; w may be overwritten
   }
 }
 
@@ -105,7 +147,7 @@ __global__ void __launch_bounds__(128) k_lu_solve(LuDev u, NewtonArgs a) {
     double s = x[(size_t)p * a.ldw];
     const int64_t d = __ldg(u.diag + p), e1 = __ldg(u.row_ptr + p + 1);
     for (int64_t e = d + 1; e < e1; ++e) s = fma(-lu[(size_t)e * a.ldw], x[(size_t)XOD_IDX(__ldg(u.col + e), u.n) * a.ldw], s);
-    x[(size_t)p * a.ldw] = s / lu[(size_t)d * a.ldw];
+    x[(size_t)p * a.ldw] = s * lu[(size_t)d * a.ldw];   // k_lu_factor stores the reciprocal of the diagonal
   }
   for (int p = 0; p < u.n; ++p) {
     const size_t sp = (size_t)XOD_IDX(__ldg(u.perm + p), u.n);

@@ -9,7 +9,10 @@
 //   * pattern: the elimination graph with fill; row p = L part | diagonal | U part in permuted indices;
 //   * schedule (row-by-row "up-looking" LU without pivoting, as DLSODES' sparse solver does): for row i
 //     and every k in L(i) ascending,  l = a_ik / a_kk;  a_ij -= l a_kj for j in U(k);  the slots of
-//     those j inside row i are precomputed (tgt).
+//     those j inside row i are precomputed (tgt);
+//   * block schedule: consecutive rows are factorised together, as many as shared memory holds; the pivots of the
+//     union of their L parts are applied in ascending order, so that a pivot's U row is read once per block and
+//     not once per row (for a trailing block that is dense, that divides the traffic by the rows per block).
 #include <algorithm>
 #include <cstring>
 
@@ -132,6 +135,45 @@ void pack_lu(HostTables &h) {
       u.rows[i] = r;
       for (int64_t x = 0; x < len; ++x) slot[u.col[b + x]] = -1;
     }
+  }
+  // block schedule: as many rows per block as shared memory holds (kLuCols columns of max_row slots each)
+  u.block_rows = (int32_t)std::min<int64_t>(kLuMaxBlockRows, (int64_t)(227 * 1024) / ((int64_t)u.max_row * kLuCols * 8));
+  if (u.block_rows < 1) {
+    u = LuHost();
+    return;
+  }
+  for (int row0 = 0; row0 < n; row0 += u.block_rows) {
+    const int nrows = std::min(u.block_rows, n - row0);
+    LuBlock blk;
+    blk.row0 = row0, blk.nrows = nrows, blk.step_begin = (int32_t)u.steps.size();
+    std::vector<size_t> cur(nrows);   // next pair of every row of the block (pairs ascend in k)
+    for (int b = 0; b < nrows; ++b) cur[b] = (size_t)u.rows[row0 + b].pair_begin;
+    for (;;) {
+      int k = -1;
+      for (int b = 0; b < nrows; ++b)
+        if (cur[b] < (size_t)u.rows[row0 + b].pair_end) {
+          const int kb = L[row0 + b][cur[b] - (size_t)u.rows[row0 + b].pair_begin];
+          if (k < 0 || kb < k) k = kb;
+        }
+      if (k < 0) break;
+      LuStep st;
+      st.diag_k = u.diag[k], st.cnt = (int32_t)U[k].size(), st.item_begin = (int32_t)u.items.size(), st.n_items = 0, st.pad = 0;
+      st.src = k >= row0 ? (k - row0) * u.max_row + (int32_t)(u.diag[k] - u.row_ptr[k]) + 1 : -1;
+      for (int b = 0; b < nrows; ++b) {
+        if (cur[b] >= (size_t)u.rows[row0 + b].pair_end) continue;
+        const size_t a = cur[b] - (size_t)u.rows[row0 + b].pair_begin;
+        if (L[row0 + b][a] != k) continue;
+        const LuPair &pr = u.pairs[cur[b]];
+        LuItem it2;
+        it2.base = b * u.max_row, it2.slot_ik = it2.base + pr.t_k, it2.tgt_off = pr.tgt_off, it2.pad = 0;
+        u.items.push_back(it2);
+        ++st.n_items, ++cur[b];
+      }
+      u.n_block_loads += st.cnt;
+      u.steps.push_back(st);
+    }
+    blk.step_end = (int32_t)u.steps.size();
+    u.blocks.push_back(blk);
   }
   u.enabled = true;
 }

@@ -142,9 +142,18 @@ struct JacTiledDev {
 // shared by all columns; values live in a [nnz_lu][cols] array, rows in elimination order, each row
 // stored as  L part (ascending) | diagonal | U part (ascending).
 constexpr int32_t kLuDiagBit = 1 << 30;   // in LuHost::src: the position is a diagonal
-constexpr int kLuWarps = 16;              // warps of a k_lu_factor CTA (32 columns x kLuWarps slices of the update loop)
+constexpr int kLuWarps = 16;              // warps of a k_lu_factor CTA
+constexpr int kLuCols = 8;                // columns per k_lu_factor CTA: a thread = (entry slice, column), 64 slices
+constexpr int kLuMaxBlockRows = 6;        // rows factorised together, all resident in shared memory
 struct LuRow { int32_t begin, len, pair_begin, pair_end; };           // storage range of the row, its (i, k) pairs
 struct LuPair { int32_t t_k, diag_k, cnt, tgt_off; };                 // slot of a_ik in row i; diagonal of row k; |U(k)|; targets
+// Block schedule of k_lu_factor: `nrows` consecutive rows sit in shared memory (row b at slot b * max_row) while the
+// pivots k of the union of their L parts are applied in ascending order; one step = one pivot, whose U row is read
+// ONCE (from global memory, or from the block's own shared rows when k is itself in the block) and applied to every
+// row of the block that holds a_ik (its items).
+struct LuBlock { int32_t row0, nrows, step_begin, step_end; };
+struct LuStep { int32_t diag_k, cnt, src, item_begin, n_items, pad; };   // src < 0: U row k in global memory from diag_k + 1; else its first shared slot
+struct LuItem { int32_t slot_ik, base, tgt_off, pad; };                  // shared slot of a_ik; first slot of the row; targets (tgt)
 struct LuHost {
   bool enabled = false;
   int32_t n = 0, max_row = 0;
@@ -155,6 +164,11 @@ struct LuHost {
   std::vector<LuRow> rows;                  // [n]
   std::vector<LuPair> pairs;                // sum_i |L(i)|, row by row, ascending k
   std::vector<uint16_t> tgt;                // for pair (i, k): slot in row i of every column of U(k)
+  int32_t block_rows = 0;                   // rows per block (<= kLuMaxBlockRows, bounded by shared memory)
+  int64_t n_block_loads = 0;                // sum over the steps of |U(k)|: U values read per column by k_lu_factor
+  std::vector<LuBlock> blocks;
+  std::vector<LuStep> steps;
+  std::vector<LuItem> items;
 };
 struct LuDev {
   int32_t enabled, n, max_row;
@@ -164,6 +178,10 @@ struct LuDev {
   const LuRow *rows;
   const LuPair *pairs;
   const uint16_t *tgt;
+  int32_t block_rows, n_blocks;
+  const LuBlock *blocks;
+  const LuStep *steps;
+  const LuItem *items;
 };
 
 // ---- tables of the pathway analyser (f4: xod_pathway; pack_path.cpp, pathway.cuh) ----------------

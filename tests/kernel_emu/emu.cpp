@@ -229,7 +229,7 @@ int emu_newton_step(const xod_network_desc *desc, int64_t ncol, int64_t ld, cons
     h.jt.enabled = false;
   }
   pack_lu(h);
-  if (!h.jt.enabled || !h.lu.enabled || (size_t)h.lu.max_row * 32 * 8 > kSmemMax) return 2;
+  if (!h.jt.enabled || !h.lu.enabled || (size_t)h.lu.block_rows * h.lu.max_row * kLuCols * 8 > kSmemMax) return 2;
   const int ns = h.ns;
   const int64_t ldw = (ncol + 31) / 32 * 32 + 32, nnzj = (int64_t)h.jac_col.size();
   std::vector<double> f((size_t)ns * ldw, NAN), rhs((size_t)ns * ldw, NAN), jac((size_t)nnzj * ldw, NAN), lu((size_t)h.lu.nnz * ldw, NAN);
@@ -260,11 +260,13 @@ int emu_newton_step(const xod_network_desc *desc, int64_t ncol, int64_t ld, cons
   ud.enabled = 1, ud.n = u.n, ud.max_row = u.max_row, ud.nnz = u.nnz;
   ud.perm = u.perm.data(), ud.diag = u.diag.data(), ud.src = u.src.data(), ud.col = u.col.data();
   ud.row_ptr = u.row_ptr.data(), ud.rows = u.rows.data(), ud.pairs = u.pairs.data(), ud.tgt = u.tgt.data();
+  ud.block_rows = u.block_rows, ud.n_blocks = (int32_t)u.blocks.size();
+  ud.blocks = u.blocks.data(), ud.steps = u.steps.data(), ud.items = u.items.data();
   NewtonArgs a{};
   a.ncol = ncol, a.ld = ld, a.ldw = ldw, a.n_old = n_old, a.dt = dt, a.f = f.data(), a.jac = jac.data();
   a.y = y, a.delta = delta, a.lu = lu.data(), a.rhs = rhs.data(), a.nnz_jac = nnzj;
   run_grid((unsigned)((ncol + 127) / 128), 3, 128, false, [&] { k_newton_assemble(ud, a); });
-  run_grid((unsigned)((ncol + 31) / 32), 1, 32 * kLuWarps, true, [&] { k_lu_factor(ud, lu.data(), ldw, ncol); });
+  run_grid((unsigned)((ncol + kLuCols - 1) / kLuCols), 1, 32 * kLuWarps, true, [&] { k_lu_factor(ud, lu.data(), ldw, ncol); });
   run_grid((unsigned)((ncol + 127) / 128), 1, 128, false, [&] { k_lu_solve(ud, a); });
   return 0;
 }
