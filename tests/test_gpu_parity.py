@@ -623,7 +623,7 @@ def test_random_networks(xod, oracle, seed):
     net.t_ref = np.where(rng.random(net.n_reactions) < 0.3, 300.0, 1.0)
     n_layers = int(rng.integers(3, 45))
     atm = synth.make_atmosphere(1900 + seed, net, 1, n_layers, t_shift=(-300.0, 300.0))
-    ncol, ld = atm.ncol, atm.ld
+    ncol, ld, ns = atm.ncol, atm.ld, net.n_species
     h = xod.Network(net, device=0)
     h.selfcheck()
     okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
