@@ -14,6 +14,27 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (runs on the B200 box)")
 
 
+# `pytest -x -m gpu` stops at the first failure: the hot path (test_gpu_parity.py) must have run
+# before any of the section 8(f) rows gets its chance to stop the session.  Everything else keeps its order.
+_GPU_ORDER = ["test_gpu_parity", "test_newton_step", "test_photo_rates", "test_transport", "test_pathway", "test_equilibrium"]
+
+
+def pytest_collection_modifyitems(session, config, items):
+    def rank(item):
+        if item.get_closest_marker("gpu") is None:
+            return -1
+        name = item.module.__name__.rsplit(".", 1)[-1]
+        r = _GPU_ORDER.index(name) if name in _GPU_ORDER else len(_GPU_ORDER)
+        # inside the hot-path file: a1-a8 (kernels that ran on a GPU in round 1) before a9's tiled Jacobian kernel
+        # (new in round 2) and before the tests that mix both
+        if "jacobian" in item.name:
+            r += 0.5
+        elif "random_networks" in item.name:
+            r += 0.6
+        return r
+    items.sort(key=rank)       # stable: the order inside a module and among the CPU tests is unchanged
+
+
 @functools.lru_cache(maxsize=None)
 def _network(cfg):
     from paper_2512_06729_b200 import synth
