@@ -27,7 +27,7 @@ def pytest_collection_modifyitems(session, config, items):
         r = _GPU_ORDER.index(name) if name in _GPU_ORDER else len(_GPU_ORDER)
         # inside the hot-path file: a1-a8 (kernels that ran on a GPU in round 1) before a9's tiled Jacobian kernel
         # (new in round 2) and before the tests that mix both
-        if "jacobian" in item.name:
+        if "jacobian" in item.name or "zero_densities" in item.name:
             r += 0.5
         elif "random_networks" in item.name:
             r += 0.6
