@@ -59,13 +59,6 @@ __device__ __noinline__ double rev_eval_other(const unsigned char *b, double T, 
   return rev_eval(b, ldg2(b + 3 * 64).y, T, l2T, invT);
 }
 
-// byte offset of the parameter block (4 reactions) that holds padded reaction pp, inside an interval
-__device__ __forceinline__ size_t block_offset(const FusedDev &f, int pp) {
-  if (pp < f.arr_end) return (size_t)(pp >> 2) * kFBlkArr;
-  if (pp < f.fo_end) return (size_t)f.blk_fo_off + (size_t)((pp - f.arr_end) >> 2) * kFBlkFo;
-  return (size_t)f.blk_ph_off + (size_t)((pp - f.fo_end) >> 2) * kFBlkPh;
-}
-
 // a7: q = k_f prod n_reactants - k_r prod n_products for the thread's two columns.  sa = the six species slots as
 // 16-bit rows of the n tile (r0 r1 | r2 p0 | p1 p2); row ns = ones (absent slot), row ns + 1 = zeros (first
 // product slot of an irreversible reaction, so that q_r = 0 exactly whatever k_r holds).
@@ -172,16 +165,25 @@ __global__ void __launch_bounds__(kFWarps * 32, 1) k_fused(FusedDev f, int ns, F
       auto passes_below = [&](int end) { const int d = end - ppw0; return d <= 0 ? 0 : min(npass, (d + kFPass - 1) / kFPass); };
       double *qdst = qb + (size_t)(warp * kFRxnPerWarp + grp) * kFW + l2;
       const int p_ph = passes_below(f.ph_end);
-      if (FROMK) {
-        const unsigned char *b = f.blk + slot16;
+      if (FROMK) {   // k_f, k_r from the caller's rows; the blocks supply the species slots only (any interval)
+        const int p_arr = passes_below(f.arr_end), p_fo = passes_below(f.fo_end);
+        const int *up = f.pp_user + ppw0 + grp;
+        auto run = [&](int pass_end, const unsigned char *b, int step, int &pass) {
 #pragma unroll 1
-        for (int pass = 0; pass < p_ph; ++pass, qdst += kFPass * kFW) {
-          const int pp = ppw0 + pass * kFPass + grp;
-          const int4 sa = __ldg(reinterpret_cast<const int4 *>(b + XOD_IDX(block_offset(f, pp), (size_t)f.blk_stride)));
-          const int user = XOD_IDX(max(__ldg(f.pp_user + pp), 0), a.nr);  // padding slots read row 0 (their q is never used)
-          const double *kfr = a.kf + (size_t)user * a.ld, *krr = a.kr + (size_t)user * a.ld;
-          rates_of_progress(sa, ns, n_l, __ldg(kfr + gc0), __ldg(kfr + gc1), __ldg(krr + gc0), __ldg(krr + gc1), qdst);
-        }
+          for (; pass < pass_end; ++pass, b += step, up += kFPass, qdst += kFPass * kFW) {
+            const int4 sa = __ldg(reinterpret_cast<const int4 *>(b));
+            const int user = XOD_IDX(max(__ldg(up), 0), a.nr);  // padding slots read row 0 (their q is never used)
+            const double *kfr = a.kf + (size_t)user * a.ld, *krr = a.kr + (size_t)user * a.ld;
+            rates_of_progress(sa, ns, n_l, __ldg(kfr + gc0), __ldg(kfr + gc1), __ldg(krr + gc0), __ldg(krr + gc1), qdst);
+          }
+        };
+        int pass = 0;
+        const unsigned char *b0 = f.blk + slot16;
+        if (p_arr > 0) run(p_arr, b0 + XOD_IDX((size_t)(ppw0 >> 2) * kFBlkArr, (size_t)f.blk_stride), kArrStep, pass);
+        if (pass < p_fo)
+          run(p_fo, b0 + XOD_IDX((size_t)f.blk_fo_off + (size_t)((ppw0 + pass * kFPass - f.arr_end) >> 2) * kFBlkFo, (size_t)f.blk_stride), kFoStep, pass);
+        if (pass < p_ph)
+          run(p_ph, b0 + XOD_IDX((size_t)f.blk_ph_off + (size_t)((ppw0 + pass * kFPass - f.fo_end) >> 2) * kFBlkPh, (size_t)f.blk_stride), kPhStep, pass);
       } else {
         const int p_arr = passes_below(f.arr_end), p_fo = passes_below(f.fo_end);
         int pass = 0;
