@@ -88,6 +88,9 @@ def test_compute_without_device_fails_loudly(built):
     st = built.xod_thermo(h._h, binding.C.c_int64(1), binding.C.c_int64(1), None, None, None, None, None, None)
     assert st == 4                                                              # XOD_ERR_CUDA, never a CPU fallback
     assert h.source_fused_workspace_bytes(150) > 0
+    C = binding.C
+    st = built.xod_equilibrium(h._h, C.c_int64(1), C.c_int64(1), None, None, None, C.c_int32(0), C.c_double(0.0), None, None, None, None)
+    assert st == 4
 
 
 def test_charge_as_an_element_and_padding_anywhere(built, oracle):
