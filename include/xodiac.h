@@ -131,7 +131,8 @@ xod_status xod_network_jac_info(const xod_network *net, int64_t *info);
 
 /* host-only consistency check of the internal tables of the fused path (decoded as the kernel
  * decodes them): every source-CSR entry and every Jacobian term scheduled exactly once, no
- * accumulator row shared by two row tasks of a chunk, species slots intact.  XOD_OK, or XOD_ERR_INVALID_ARG with xod_last_error. */
+ * accumulator row shared by two row tasks of a chunk, species slots intact; with XOD_FLAG_BUILD_LU also the
+ * implicit step's rows, target slots and block schedule (every (row, pivot) pair applied exactly once, pivots ascending).  XOD_OK, or XOD_ERR_INVALID_ARG with xod_last_error. */
 xod_status xod_network_selfcheck(const xod_network *net);
 
 /* ---- tuning knobs (optional; defaults are chosen for B200) */

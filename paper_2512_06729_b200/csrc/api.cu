@@ -434,6 +434,7 @@ xod_status xod_network_selfcheck(const xod_network *net) {
   std::string err;
   if (!check_fused(net->h, err)) return fail(XOD_ERR_INVALID_ARG, err);
   if (!check_jac_tiled(net->h, err)) return fail(XOD_ERR_INVALID_ARG, err);
+  if (!check_lu(net->h, err)) return fail(XOD_ERR_INVALID_ARG, err);
   return XOD_OK;
 }
 

@@ -179,3 +179,88 @@ void pack_lu(HostTables &h) {
 }
 
 }  // namespace xod
+
+namespace xod {
+
+// Host-only self-check of the implicit-step tables, decoding them exactly as the kernels of newton.cuh do:
+//  * rows tile the value array; the diagonal sits after the L part; columns ascend; L(i) < i < U(i);
+//  * every pair (i, k) names a slot of row i that holds column k, the diagonal of row k, |U(k)| targets, and every
+//    target slot of row i holds the column of the matching entry of U(k);
+//  * the block schedule covers the rows in order, at most block_rows at a time, within shared memory; every pair
+//    of a block's rows appears exactly once as an item, under a step of its own pivot, steps ascending in the pivot;
+//    a pivot inside the block is read from the shared slot right after that row's diagonal, a pivot before the
+//    block from global memory.
+bool check_lu(const HostTables &h, std::string &err) {
+  const LuHost &u = h.lu;
+  if (!u.enabled) return true;
+  auto fail = [&](const std::string &m) { err = "LU tables: " + m; return false; };
+  const int n = u.n;
+  if ((int)u.rows.size() != n || (int)u.diag.size() != n || (int)u.row_ptr.size() != n + 1) return fail("sizes");
+  std::vector<int32_t> row_of_diag(u.nnz, -1);
+  for (int i = 0; i < n; ++i) {
+    const LuRow &r = u.rows[i];
+    if (r.begin != u.row_ptr[i] || r.len != u.row_ptr[i + 1] - u.row_ptr[i] || r.len > u.max_row) return fail("row range");
+    const int n_l = r.pair_end - r.pair_begin;
+    if (u.diag[i] != r.begin + n_l || u.col[u.diag[i]] != i) return fail("diagonal position");
+    for (int t = 0; t < r.len; ++t) {
+      const int c = u.col[r.begin + t];
+      if (c < 0 || c >= n || (t > 0 && c <= u.col[r.begin + t - 1])) return fail("columns not ascending");
+      if ((t < n_l) != (c < i)) return fail("L / U split");
+    }
+    row_of_diag[u.diag[i]] = i;
+  }
+  for (int i = 0; i < n; ++i) {
+    const LuRow &r = u.rows[i];
+    for (int p = r.pair_begin; p < r.pair_end; ++p) {
+      const LuPair &pr = u.pairs[p];
+      if (pr.t_k != p - r.pair_begin || pr.diag_k < 0 || pr.diag_k >= u.nnz || row_of_diag[pr.diag_k] < 0) return fail("pair");
+      const int k = row_of_diag[pr.diag_k];
+      if (u.col[r.begin + pr.t_k] != k) return fail("pair slot does not hold its pivot column");
+      const int64_t ub = (int64_t)u.diag[k] + 1, ue = u.row_ptr[k + 1];
+      if (pr.cnt != ue - ub || (int64_t)pr.tgt_off + pr.cnt > (int64_t)u.tgt.size()) return fail("pair count");
+      for (int jj = 0; jj < pr.cnt; ++jj) {
+        const int slot = u.tgt[(size_t)pr.tgt_off + jj];
+        if (slot >= r.len || u.col[r.begin + slot] != u.col[ub + jj]) return fail("target slot holds another column");
+      }
+    }
+  }
+  if (u.block_rows < 1 || u.block_rows > kLuMaxBlockRows || (int64_t)u.block_rows * u.max_row * kLuCols * 8 > 227 * 1024)
+    return fail("block rows");
+  int next_row = 0;
+  std::vector<char> seen(u.pairs.size(), 0);
+  for (const LuBlock &b : u.blocks) {
+    if (b.row0 != next_row || b.nrows < 1 || b.nrows > u.block_rows || b.row0 + b.nrows > n) return fail("block range");
+    next_row += b.nrows;
+    int last_k = -1;
+    for (int si = b.step_begin; si < b.step_end; ++si) {
+      const LuStep &st = u.steps[(size_t)si];
+      if (st.diag_k < 0 || st.diag_k >= u.nnz || row_of_diag[st.diag_k] < 0) return fail("step pivot");
+      const int k = row_of_diag[st.diag_k];
+      if (k <= last_k) return fail("steps not ascending in the pivot");
+      last_k = k;
+      if (st.cnt != u.row_ptr[k + 1] - u.diag[k] - 1 || st.n_items < 1 || st.n_items > b.nrows) return fail("step");
+      const int want_src = k >= b.row0 ? (k - b.row0) * u.max_row + (int)(u.diag[k] - u.row_ptr[k]) + 1 : -1;
+      if (st.src != want_src || k >= b.row0 + b.nrows) return fail("step source");
+      for (int x = 0; x < st.n_items; ++x) {
+        const LuItem &it = u.items[(size_t)st.item_begin + x];
+        if (it.base % u.max_row != 0) return fail("item base");
+        const int brow = it.base / u.max_row;
+        if (brow < 0 || brow >= b.nrows) return fail("item row");
+        const int i = b.row0 + brow;
+        if (i <= k) return fail("item row does not lie below its pivot");
+        const LuRow &r = u.rows[i];
+        const int t_k = it.slot_ik - it.base;
+        if (t_k < 0 || t_k >= r.pair_end - r.pair_begin) return fail("item slot");
+        const int p = r.pair_begin + t_k;
+        if (u.pairs[p].diag_k != st.diag_k || u.pairs[p].tgt_off != it.tgt_off || seen[p]) return fail("item does not match its pair");
+        seen[p] = 1;
+      }
+    }
+  }
+  if (next_row != n) return fail("blocks do not cover the rows");
+  for (char c : seen)
+    if (!c) return fail("a (row, pivot) pair is missing from the block schedule");
+  return true;
+}
+
+}  // namespace xod

@@ -258,6 +258,7 @@ void pack_jac_tiled(HostTables &h, int chunk, int acc_budget);
 bool check_jac_tiled(const HostTables &h, std::string &err);
 // pack_lu.cpp: minimum-degree ordering, filled pattern and update schedule of the implicit step
 void pack_lu(HostTables &h);
+bool check_lu(const HostTables &h, std::string &err);
 // pack_path.cpp: incoming-edge lists and step schedule of the pathway analyser
 void pack_path(const xod_network_desc *d, HostTables &h);
 size_t path_smem_bytes(int ns);

@@ -97,6 +97,12 @@ def test_symbolic_lu_is_the_elimination_closure_of_the_jacobian_pattern(network,
     assert info["nnz_lu"] == int(m.sum()) and info["max_row"] == int(m.sum(axis=1).max())
     assert info["updates"] == sum(int(m[k + 1:, k].sum()) * int(m[k, k + 1:].sum()) for k in range(ns))
     print("config %d: nnz(Jac) %d -> nnz(L+U) %d, %d multiply-add updates per factorisation" % (cfg, jcol.size, info["nnz_lu"], info["updates"]))
+    # the update and block schedules, decoded on the host as k_lu_factor decodes them: every (row, pivot) pair once,
+    # pivots ascending inside a block, target slots holding the right columns
+    h.selfcheck()
+    assert 1 <= info["block_rows"] <= 6 and info["steps"] <= info["pairs"]
+    # a pivot's U row is read once per block instead of once per row: between updates / block_rows and updates
+    assert info["updates"] / info["block_rows"] <= info["u_loads"] <= info["updates"]
 
 
 def test_networks_without_the_flag_have_no_lu_tables(network):
