@@ -419,6 +419,11 @@ net2 = synth.config_network(2)
 atm2 = synth.config_atmosphere(2, net2)
 k2 = np.full((net2.n_reactions, atm2.ld), 1e-12)
 tpw.run_emulated(net2, k2, k2, atm2.n, 37, atm2.ld, 5, 2)
+import test_equilibrium as teq
+comp2 = np.asarray(net2.composition, dtype=np.float64)
+b2 = np.ascontiguousarray(comp2.T @ atm2.n)
+n_eq, pi_eq, it_eq = teq.run_emulated(net2, np.ascontiguousarray(atm2.T), np.ascontiguousarray(atm2.P), b2, 37, atm2.ld)
+assert np.all(it_eq[:37] > 0)
 print("emulated-ok")
 """
 
