@@ -269,6 +269,14 @@ def stage_timings(binding, h3, net, dev, ws_for, dfma_per_s):
             tot += event_time_ms(fn, 1, sync)
         return tot / reps
 
+    # context for the write-bound stages (xod_thermo, xod_rate_coeffs, xod_jacobian): MEASURED_PEAKS.json's HBM figure is a
+    # copy (read + write bytes); a pure write stream has its own ceiling, probed here with a device fill of 256 MB
+    try:
+        for _ in range(3):
+            flush.fill_(0)
+        out["hbm_write_only_gbs"] = flush.numel() / (event_time_ms(lambda: flush.fill_(1), 10, sync) * 1e-3) / 1e9
+    except Exception as exc:
+        out["hbm_write_only_gbs"] = {"error": repr(exc)[:200]}
     for cfg, reps in ((3, 200), (5, 5)):
         atm = synth.config_atmosphere(cfg, net)
         ncol, ld = atm.ncol, atm.ld
