@@ -169,3 +169,38 @@ def test_an_element_without_abundance_is_refused(oracle):
     net = simple([[1, 0], [0, 1]], [-1.0, -1.0])
     with pytest.raises(ArithmeticError):
         oracle.equilibrium(net, np.array([1000.0]), np.array([1e6]), np.array([[1.0], [0.0]]))
+
+
+def test_a_general_purpose_minimiser_finds_the_same_composition(oracle):
+    """A different algorithm on the same definition: scipy's SLSQP minimises G/RT over the mole numbers under the
+    linear element constraints (no Lagrange iteration, no logarithmic variables) for a 5-species, 2-element gas;
+    it converges to about 1e-7, the oracle must agree with it to that accuracy."""
+    from scipy.optimize import minimize
+    comp = np.array([[1, 0], [0, 1], [2, 0], [1, 1], [2, 1]], dtype=float)     # A, B, A2, AB, A2B
+    gs = np.array([-1.0, -2.0, -6.5, -7.0, -11.0])
+    net = simple(comp.astype(int).tolist(), gs.tolist())
+    T, P = np.array([1200.0]), np.array([3.0e5])
+    b = np.array([[2.0], [1.0]])
+    n, it = oracle.equilibrium(net, T, P, b)
+    x = n[:, 0] / n[:, 0].sum()
+    p = P[0] / P0
+
+    def G(m):
+        m = np.maximum(m, 1e-300)
+        return float(np.sum(m * (gs + np.log(m / m.sum()) + np.log(p))))
+
+    cons = {"type": "eq", "fun": lambda m: comp.T @ m - b[:, 0], "jac": lambda m: comp.T}
+    best = None
+    for seed in range(4):
+        m0 = np.random.default_rng(seed).uniform(0.05, 0.5, 5)
+        r = minimize(G, m0, method="SLSQP", constraints=[cons], bounds=[(1e-12, None)] * 5,
+                     options={"ftol": 1e-15, "maxiter": 500})
+        if r.success and (best is None or r.fun < best.fun):
+            best = r
+    assert best is not None
+    xs = best.x / best.x.sum()
+    assert np.allclose(xs, x, rtol=0, atol=2e-6), (xs, x)
+    # and the oracle's point is at least as low as the minimiser's, on the minimiser's own scale
+    m_or = x * (b[0, 0] / (comp[:, 0] @ x))
+    assert np.allclose(comp.T @ m_or, b[:, 0], rtol=1e-13)
+    assert G(m_or) <= best.fun + 1e-9 * abs(best.fun)
