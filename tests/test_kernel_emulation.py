@@ -514,3 +514,29 @@ def test_random_networks_through_the_kernel_sources(emu, oracle, seed):
     G.check_sum_entries(jac, wj, sj, ncol, "random net %d k_jac_tiled" % seed)
     print("random network %d: %d species, %d reactions (%d irreversible), %d columns: ok" % (
         seed, net.n_species, net.n_reactions, int((net.reversible == 0).sum()), ncol))
+
+
+def test_kernel_sources_at_the_ends_of_the_temperature_range(emu, oracle, network):
+    """the network is "valid" from 100 K to 30 000 K, far outside the 200-3000 K of the thermo fits
+    (reading T4: extrapolate, no clamp).  Columns at 100, 120, 3 000, 10 000 and 30 000 K: most reverse coefficients
+    over- or underflow at the cold end and the extrapolated quartic does at the hot end (reading R5 decides what the
+    kernels must return there); everything in between must match to 1e-12."""
+    from paper_2512_06729_b200 import synth
+    net = network(2)
+    atm = synth.make_atmosphere(2077, net, 1, 20)
+    atm.T[:20] = np.array([100.0, 120.0, 150.0, 200.0, 3000.0, 5000.0, 10000.0, 20000.0, 30000.0, 30000.0] * 2)
+    ncol, ld = atm.ncol, atm.ld
+    d, keep = descriptor(net)
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    kf, kr = np.full((net.n_reactions, ld), np.nan), np.full((net.n_reactions, ld), np.nan)
+    assert emu.emu_rate_coeffs(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J), ptr(kf), ptr(kr),
+                               C.c_int(16)) == 0
+    worst_f = G.check_k(kf[:, :ncol], okf[:, :ncol], "k_f at the ends of the range")
+    worst_r = G.check_k(kr[:, :ncol], okr[:, :ncol], "k_r at the ends of the range")
+    cold, hot = atm.T[:ncol] <= 200.0, atm.T[:ncol] >= 10000.0      # both ends leave the double range for some reactions:
+    assert np.isinf(okr[:, :ncol][:, cold]).any() and np.isinf(okr[:, :ncol][:, hot]).any()   # a6 / T when cold, a5 T^4 when hot
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    got = run_fused(emu, net, atm, ncol, grid=2, nsplit=1)
+    worst, skipped = G.check_sum_entries(got, want, wp + wl, ncol, "k_fused at the ends of the range")
+    print("100 K .. 30 000 K: worst relative error k_f %.2e, k_r %.2e; dn/dt %.2e of scale, %d non-finite entries skipped"
+          % (worst_f, worst_r, worst, skipped))
