@@ -105,3 +105,24 @@ def test_photo_create_validates_its_tables(network):
     bad2.sigma_ph[0, 0] = -1.0
     with pytest.raises(binding.XodError):
         binding.Photo(h, bad2)
+
+
+@pytest.mark.parametrize("n_abs,n_layers,n_bins", [(0, 7, 5), (3, 1, 33), (2, 40, 1)])
+def test_emulated_photo_rates_degenerate_shapes(oracle, network, n_abs, n_layers, n_bins):
+    """No absorber at all (a transparent atmosphere: the contraction over absorbers has K = 0), atmospheres of a
+    single layer (tau = half the layer's own slab), a single wavelength bin."""
+    from paper_2512_06729_b200 import synth
+    net = network(1)
+    atm = synth.make_atmosphere(2301, net, 3, n_layers)
+    ph = synth.make_photo(77, net, n_bins=n_bins, n_abs=max(n_abs, 1))
+    if n_abs == 0:
+        ph.abs_species = np.zeros(0, dtype=np.int32)
+        ph.sigma_ext = np.zeros((0, n_bins))
+    dz, j0, jd, mu, tf = synth.make_irradiation(78, net, atm, ph, with_diffuse=False)
+    want = oracle.photo_rates(ph, atm.n, dz, j0, jd, mu, tf, 3, n_layers)
+    got = run_emulated(net, atm, ph, dz, j0, jd, mu, tf)
+    check(got, want, atm.ncol, "emulated xod_photo_rates, %d absorbers, %d layers, %d bins" % (n_abs, n_layers, n_bins))
+    if n_abs == 0:      # transparent: k_ph = t_f sum_b J0 sigma dlambda in every layer (PAPER.md:207 with tau = 0)
+        flat = (np.asarray(tf)[:, None] * (np.asarray(j0) * ph.dlambda[None, :]) @ ph.sigma_ph.T)     # [atm][photo]
+        for a in range(3):
+            assert np.allclose(got[:, a * n_layers:(a + 1) * n_layers], flat[a][:, None], rtol=1e-12, atol=0)
