@@ -50,7 +50,7 @@ def check(got, want, S, ncol, what):
     assert np.all(err <= 1e-12 * S[:, :ncol]), "%s: worst ratio %.2e" % (what, float((err / np.maximum(S[:, :ncol], 1e-300)).max()))
     assert np.all(np.isnan(got[:, ncol:])), what + ": padding columns written"
     nz = S[:, :ncol] > 0
-    print("%s: %d x %d values, worst |err| / sum|terms| = %.2e" % (what, got.shape[0], ncol, float((err[nz] / S[:, :ncol][nz]).max())))
+    print("%s: %d x %d values, worst |err| / sum|terms| = %.2e" % (what, got.shape[0], ncol, float((err[nz] / S[:, :ncol][nz]).max()) if nz.any() else 0.0))
 
 
 def oracle_tr(oracle, atm, t):
@@ -94,3 +94,25 @@ def test_transport_matches_oracle_on_gpu(oracle, network, cfg, n_atm):
     h.check_status()
     check(G.host(tr), want, scale(net, atm, t), atm.ncol, "xod_transport config %d, %d atmospheres" % (cfg, n_atm))
     h.close()
+
+
+@pytest.mark.parametrize("n_layers", [1, 2, 3])
+def test_emulated_transport_on_the_thinnest_atmospheres(oracle, network, n_layers):
+    """One layer (both boundaries at once: no term survives), two layers (every layer touches a
+    boundary) and three; five atmospheres side by side, so neighbours in memory belong to other atmospheres."""
+    import test_kernel_emulation as tk
+    from paper_2512_06729_b200 import synth
+    net = network(1)
+    atm = synth.make_atmosphere(2401, net, 5, n_layers)
+    t = synth.make_transport(62, net, atm)
+    want = oracle_tr(oracle, atm, t)
+    lib = C.CDLL(tk.LIB)
+    got = np.full((net.n_species, atm.ld), np.nan)
+    c = lambda a: np.ascontiguousarray(a, dtype=np.float64)
+    arrs = [c(atm.n), c(atm.T), c(t["n_gas"]), c(t["D"]), c(t["mass"]), c(t["alpha_T"]), c(t["mbar"]), c(t["grav"]), c(t["dz"])]
+    rc = lib.emu_transport(C.c_int(net.n_species), C.c_int64(5), C.c_int64(n_layers), C.c_int64(atm.ld),
+                           *[tk.ptr(x) for x in arrs], tk.ptr(got), C.c_int(4))
+    assert rc == 0
+    check(got, want, scale(net, atm, t), atm.ncol, "emulated xod_transport, %d layer(s)" % n_layers)
+    if n_layers == 1:
+        assert np.all(got[:, :atm.ncol] == 0.0)
