@@ -657,3 +657,38 @@ def test_random_networks(xod, oracle, seed):
         G.check_sum_entries(G.host(jac), wj, sj, ncol, "random net %d xod_jacobian (tiled %d)" % (seed, tiled))
     h.check_status()
     h.close()
+
+
+def test_network_too_large_for_the_fused_tables_and_its_jacobian(xod, oracle):
+    """950 species: k_fused's tiles do not fit shared memory, so every call must take the multi-kernel pipeline
+    (xod_network_fused_info says so); the tiled Jacobian still fits.  Ragged column count."""
+    from paper_2512_06729_b200 import synth
+    net = synth.make_network(777, ["H", "C", "O", "N", "S"], 950, 300, inert=())
+    atm = synth.make_atmosphere(2777, net, 1, 19)
+    h = xod.Network(net, device=0)
+    assert h.fused_info()["enabled"] == 0 and h.jac_info()["enabled"] == 1
+    ns, ld, ncol = net.n_species, atm.ld, atm.ncol
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    dT, dP, dJ, dn = (G.dev(a) for a in (atm.T, atm.P, atm.J, atm.n))
+    ws = G.workspace(max(h.source_fused_workspace_bytes(ncol), h.source_workspace_bytes(ncol), h.rate_coeffs_workspace_bytes(ncol)))
+    kf, kr = G.empty(net.n_reactions, ld), G.empty(net.n_reactions, ld)
+    h.rate_coeffs(ncol, ld, dT, dP, dJ, kf, kr, ws)
+    G.check_k(G.host(kf)[:, :ncol], okf[:, :ncol], "950 species k_f")
+    G.check_k(G.host(kr)[:, :ncol], okr[:, :ncol], "950 species k_r")
+    cols = np.arange(ncol)
+    d0, p0, l0 = G.empty(ns, ld), G.empty(ns, ld), G.empty(ns, ld)
+    h.source_fused(ncol, ld, dT, dP, dJ, dn, d0, p0, l0, workspace=ws)
+    G.check_sum(G.host(d0), want, wp + wl, cols, "950 species dn/dt")
+    G.check_sum(G.host(p0), wp, wp + wl, cols, "950 species P")
+    G.check_sum(G.host(l0), wl, wp + wl, cols, "950 species L")
+    d1 = G.empty(ns, ld)
+    h.source(ncol, ld, G.dev(okf), G.dev(okr), dn, d1, workspace=ws)
+    G.check_sum(G.host(d1), want, wp + wl, cols, "950 species dn/dt from stored k")
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
+    jac = G.empty(h.nnz_jac, ld)
+    h.jacobian(ncol, ld, G.dev(okf), G.dev(okr), dn, jac)
+    G.check_sum(G.host(jac), wj, sj, cols, "950 species Jacobian")
+    h.check_status()
+    h.close()

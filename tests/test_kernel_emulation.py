@@ -540,3 +540,37 @@ def test_kernel_sources_at_the_ends_of_the_temperature_range(emu, oracle, networ
     worst, skipped = G.check_sum_entries(got, want, wp + wl, ncol, "k_fused at the ends of the range")
     print("100 K .. 30 000 K: worst relative error k_f %.2e, k_r %.2e; dn/dt %.2e of scale, %d non-finite entries skipped"
           % (worst_f, worst_r, worst, skipped))
+
+
+def test_a_network_too_large_for_the_single_kernel_tables(emu, oracle):
+    """950 species: the n tile and the accumulator tile of k_fused no longer fit one CTA's shared memory together, so
+    the library must disable the fused tables (xod_network_fused_info) and serve xod_rate_coeffs / xod_source /
+    xod_source_fused by the multi-kernel pipeline; the tiled Jacobian (one accumulator set per unit only) still fits.
+    Both are run here against the oracle, with a ragged column count."""
+    from paper_2512_06729_b200 import synth
+    net = synth.make_network(777, ["H", "C", "O", "N", "S"], 950, 300, inert=())
+    atm = synth.make_atmosphere(2777, net, 1, 19)
+    h = binding.Network(net, device=-1)
+    assert h.fused_info()["enabled"] == 0 and h.jac_info()["enabled"] == 1
+    h.selfcheck()
+    d, keep = descriptor(net)
+    ns, ld, ncol = net.n_species, atm.ld, atm.ncol
+    okf, okr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    want, wp, wl = oracle.source(net, okf, okr, atm.n, ncol)
+    kf, kr = np.full((net.n_reactions, ld), np.nan), np.full((net.n_reactions, ld), np.nan)
+    assert emu.emu_rate_coeffs_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J),
+                                        ptr(kf), ptr(kr), C.c_int(16)) == 0
+    G.check_k(kf[:, :ncol], okf[:, :ncol], "950 species k_f")
+    G.check_k(kr[:, :ncol], okr[:, :ncol], "950 species k_r")
+    dn, pr, lo = (np.full((ns, ld), np.nan) for _ in range(3))
+    assert emu.emu_source_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(atm.T), ptr(atm.P), ptr(atm.J), None, None,
+                                   ptr(atm.n), ptr(dn), ptr(pr), ptr(lo), C.c_int(16)) == 0
+    check(dn, want, wp + wl, ncol, "950 species dn/dt")
+    check(pr, wp, wp + wl, ncol, "950 species P")
+    check(lo, wl, wp + wl, ncol, "950 species L")
+    rp, col = h.jac_pattern()
+    wj, sj = oracle.jacobian(net, okf, okr, atm.n, rp, col, ncol)
+    jac = np.full((col.shape[0], ld), np.nan)
+    assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr), ptr(atm.n), ptr(jac),
+                                  C.c_int(2), C.c_int(2)) == 0
+    G.check_sum(jac, wj, sj, np.arange(ncol), "950 species k_jac_tiled")
