@@ -692,3 +692,32 @@ def test_network_too_large_for_the_fused_tables_and_its_jacobian(xod, oracle):
     G.check_sum(G.host(jac), wj, sj, cols, "950 species Jacobian")
     h.check_status()
     h.close()
+
+
+def test_network_without_reactions_and_its_jacobian(xod):
+    """The empty reaction list: dn/dt, P, L and the Jacobian (pattern = the diagonal) are exact zeros; xod_rate_coeffs
+    has nothing to write; padding columns stay untouched."""
+    import torch
+    from conftest import SimpleNet
+    net = SimpleNet([[1], [2], [1]], np.zeros((3, 7)), np.zeros((3, 7)), [1000.0] * 3, [], [], [], [], np.zeros((0, 3)))
+    h = xod.Network(net, device=0)
+    ncol, ld = 37, 64
+    T, P = G.dev(np.full(ld, 1200.0)), G.dev(np.full(ld, 1e5))
+    n = G.dev(np.abs(np.random.default_rng(3).normal(size=(3, ld))) * 1e10)
+    ws = G.workspace(max(h.source_fused_workspace_bytes(ncol), h.source_workspace_bytes(ncol)) + 4096)
+    for pl in (False, True):
+        d0, p0, l0 = G.empty(3, ld), G.empty(3, ld), G.empty(3, ld)
+        h.source_fused(ncol, ld, T, P, None, n, d0, p0 if pl else None, l0 if pl else None, workspace=ws)
+        outs = (d0, p0, l0) if pl else (d0,)
+        for a in outs:
+            got = G.host(a)
+            assert np.all(got[:, :ncol] == 0.0) and np.all(np.isnan(got[:, ncol:]))
+        d1 = G.empty(3, ld)
+        h.source(ncol, ld, None, None, n, d1, workspace=ws)
+        assert np.all(G.host(d1)[:, :ncol] == 0.0)
+    jac = G.empty(h.nnz_jac, ld)
+    h.jacobian(ncol, ld, None, None, n, jac)
+    got = G.host(jac)
+    assert h.nnz_jac == 3 and np.all(got[:, :ncol] == 0.0) and np.all(np.isnan(got[:, ncol:]))
+    h.check_status()
+    h.close()

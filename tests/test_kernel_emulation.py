@@ -574,3 +574,26 @@ def test_a_network_too_large_for_the_single_kernel_tables(emu, oracle):
     assert emu.emu_jacobian_tiled(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(okf), ptr(okr), ptr(atm.n), ptr(jac),
                                   C.c_int(2), C.c_int(2)) == 0
     G.check_sum(jac, wj, sj, np.arange(ncol), "950 species k_jac_tiled")
+
+
+def test_a_network_without_reactions(emu):
+    """The empty reaction list: dn/dt, P and L are exact zeros for every species and the Jacobian (its pattern is the
+    diagonal alone) is zero too; nothing outside the asked columns is written."""
+    from conftest import SimpleNet
+    net = SimpleNet([[1], [2], [1]], np.zeros((3, 7)), np.zeros((3, 7)), [1000.0] * 3, [], [], [], [], np.zeros((0, 3)))
+    h = binding.Network(net, device=-1)
+    assert h.fused_info()["enabled"] == 0 and h.jac_info()["enabled"] == 0 and h.nnz_jac == 3
+    d, keep = descriptor(net)
+    ncol, ld = 37, 64
+    T, P = np.full(ld, 1200.0), np.full(ld, 1e5)
+    J = np.zeros((0, ld))
+    n = np.abs(np.random.default_rng(3).normal(size=(3, ld))) * 1e10
+    dn, pr, lo = (np.full((3, ld), np.nan) for _ in range(3))
+    assert emu.emu_source_pipeline(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(T), ptr(P), ptr(J), None, None, ptr(n), ptr(dn),
+                                   ptr(pr), ptr(lo), C.c_int(16)) == 0
+    for a in (dn, pr, lo):
+        assert np.all(a[:, :ncol] == 0.0) and np.all(np.isnan(a[:, ncol:]))
+    jac = np.full((3, ld), np.nan)
+    empty = np.zeros((0, ld))
+    assert emu.emu_jacobian(C.byref(d), C.c_int64(ncol), C.c_int64(ld), ptr(empty), ptr(empty), ptr(n), ptr(jac), C.c_int(3)) == 0
+    assert np.all(jac[:, :ncol] == 0.0) and np.all(np.isnan(jac[:, ncol:]))
