@@ -278,3 +278,42 @@ def test_double_build_of_source_agrees(oracle, oracle_f64, network):
     scale = a[1] + a[2]
     # k_r in pure double carries |dG/RT| * 2^-53 relative error (~1e-13 at these temperatures)
     assert np.all(np.abs(a[0] - b[0]) <= 5e-12 * scale)
+
+
+@pytest.mark.parametrize("seed", [11, 13, 16])
+def test_invariants_on_random_networks_with_one_way_reactions(oracle, seed):
+    """The conservation laws do not care which reactions are reversible or which rate form they use: on seeded random
+    networks with 30 % one-way thermal reactions and Kooij forms mixed in (the networks of the kernel tests), dn/dt
+    conserves every element, so does every Jacobian column, one-way reactions have k_r = 0 exactly, and reversible
+    ones obey k_f / k_r = K_c rebuilt here from the thermo output."""
+    from paper_2512_06729_b200 import synth
+    rng = np.random.default_rng(seed)
+    elements = ["H", "C", "O", "N", "S"][:int(rng.integers(2, 6))]
+    ns = int(rng.integers(6, 40))
+    nr = int(rng.integers(5, 330))
+    net = synth.make_network(900 + seed, elements, ns, nr, inert=())
+    flip = rng.random(net.n_reactions) < 0.3
+    net.reversible = np.where(flip & (net.type != 3), 0, net.reversible).astype(np.uint8)
+    net.t_ref = np.where(rng.random(net.n_reactions) < 0.3, 300.0, 1.0)
+    atm = synth.make_atmosphere(1900 + seed, net, 1, 12)
+    ncol = atm.ncol
+    kf, kr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
+    assert np.all(kr[net.reversible == 0, :ncol] == 0.0) and np.all(kr[net.reversible == 1, :ncol] > 0.0)
+    g = oracle.thermo(net, atm.T, ncol)[3]
+    kB, P0 = 1.380649e-16, 1.0e6
+    for r in np.flatnonzero(net.reversible == 1)[:40]:
+        dg = sum(g[s] for s in net.products[r] if s >= 0) - sum(g[s] for s in net.reactants[r] if s >= 0)
+        dnu = int((net.products[r] >= 0).sum()) - int((net.reactants[r] >= 0).sum())
+        kc = np.exp(-dg[:ncol]) * (P0 / (kB * atm.T[:ncol])) ** dnu
+        assert np.allclose(kf[r, :ncol] / kr[r, :ncol], kc, rtol=1e-11, atol=0)
+    dndt, prod, loss = oracle.source(net, kf, kr, atm.n, ncol)
+    res, ref = _element_residual(net, dndt[:, :ncol], (prod + loss)[:, :ncol])
+    assert np.all(np.abs(res) <= 1e-15 * ref)
+    row_ptr, col = oracle.jac_pattern(net)
+    jac, sc = oracle.jacobian(net, kf, kr, atm.n, row_ptr, col, 3)
+    a = net.composition.astype(np.float64)
+    rows = np.repeat(np.arange(net.n_species), np.diff(row_ptr))
+    for c in range(3):
+        dense, scale = np.zeros((net.n_species,) * 2), np.zeros((net.n_species,) * 2)
+        dense[rows, col], scale[rows, col] = jac[:, c], sc[:, c]
+        assert np.all(np.abs(a.T @ dense) <= 1e-15 * (np.abs(a).T @ scale))
