@@ -84,6 +84,30 @@ def test_emulated_equilibrium_matches_oracle(oracle, network, cfg, ncol_max, shi
     check(net, T, P, b, ncol, got, want, "emulated xod_equilibrium config %s (T shift %+.0f K)" % (cfg, shift))
 
 
+def coldest_config4_atmosphere(network):
+    """The coldest of the 256 atmospheres of config 4 (T down to ~175 K at the top, |G/RT| of several hundred)."""
+    from paper_2512_06729_b200 import synth
+    net = network(3)
+    atm = synth.config_atmosphere(4, net)
+    a = int(np.argmin(atm.T[:atm.ncol])) // 150
+    sl = slice(a * 150, (a + 1) * 150)
+    ncol, ld = 150, 160
+    T, P = np.full(ld, 1000.0), np.full(ld, 1.0e6)
+    T[:150], P[:150] = atm.T[sl], atm.P[sl]
+    n0 = np.ones((net.n_species, ld))
+    n0[:, :150] = atm.n[:, sl]
+    b = np.ascontiguousarray(np.asarray(net.composition, dtype=np.float64).T @ n0)
+    return net, T, P, b, ncol, ld
+
+
+def test_emulated_equilibrium_on_the_coldest_atmosphere_of_config_4(oracle, network):
+    net, T, P, b, ncol, ld = coldest_config4_atmosphere(network)
+    assert T[:ncol].min() < 200.0
+    want = oracle.equilibrium(net, T, P, b, ncol)
+    got = run_emulated(net, T, P, b, ncol, ld)
+    check(net, T, P, b, ncol, got, want, "emulated xod_equilibrium, coldest atmosphere of config 4")
+
+
 def test_emulated_equilibrium_reports_rejected_and_unconverged_columns(network):
     """Column 1 has a missing element, column 2 a negative temperature: iters = 0 and NaN; with max_iter = 3 nothing
     converges: iters = -3 and NaN; the other columns are unaffected by their neighbours."""
@@ -102,13 +126,13 @@ def test_emulated_equilibrium_reports_rejected_and_unconverged_columns(network):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg,ncol_max,shift", [(1, 20, 0.0), (2, 120, 0.0), (2, 120, -550.0), ("edge", 75, 0.0), (3, 150, 0.0),
-                                                (4, 450, 0.0)])
+                                                (4, 450, 0.0), ("cold4", 150, 0.0)])
 def test_equilibrium_matches_oracle_on_gpu(oracle, network, cfg, ncol_max, shift):
     import torch
     assert torch.cuda.is_available(), "no CUDA device: the gpu tests need the B200 box (there is no CPU fallback)"
     from paper_2512_06729_b200 import binding, build
     build.build()
-    net, T, P, b, ncol, ld = case(network, cfg, ncol_max, shift)
+    net, T, P, b, ncol, ld = coldest_config4_atmosphere(network) if cfg == "cold4" else case(network, cfg, ncol_max, shift)
     want = oracle.equilibrium(net, T, P, b, ncol)
     h = binding.Network(net, device=0)
     ne = np.asarray(net.composition).shape[1]
