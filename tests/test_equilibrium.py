@@ -57,6 +57,20 @@ def check(net, T, P, b, ncol, got, want, what):
         what, ncol, iters[:ncol].min(), iters[:ncol].max(), wit[:ncol].min(), wit[:ncol].max(), worst, ratio_err))
 
 
+def touched_by_underflow(net, n, ncol):
+    """[species][column] mask: the species takes part in a reaction one of whose participants has an equilibrium
+    density below the double range in that column.  There the balance q_f = q_r holds mathematically (k_r ~ 1e260
+    times n ~ 1e-380) but cannot be formed in fp64 (n is returned as 0), so the kinetic cross-check skips it."""
+    tiny = n[:, :ncol] < 1e-280
+    out = np.zeros_like(tiny)
+    for r in range(net.n_reactions):
+        sp = [s for s in list(net.reactants[r]) + list(net.products[r]) if s >= 0]
+        bad = tiny[sp].any(axis=0)
+        for s in sp:
+            out[s] |= bad
+    return out
+
+
 def run_emulated(net, T, P, b, ncol, ld, max_iter=0, tol=0.0):
     import os
     import subprocess
@@ -142,6 +156,9 @@ def test_equilibrium_matches_oracle_on_gpu(oracle, network, cfg, ncol_max, shift
     h.check_status()
     got = (G.host(n), G.host(pi), iters.cpu().numpy())
     check(net, T, P, b, ncol, got, want, "xod_equilibrium config %s (T shift %+.0f K)" % (cfg, shift))
+    if np.any((np.asarray(net.reversible) == 0) & (np.asarray(net.type) != 3)):
+        h.close()
+        return        # one-way thermal reactions (the edge network) are not balanced at equilibrium: no kinetic cross-check
     # the kinetics agree: without photolysis dn/dt vanishes at the returned composition (xod_source_fused vs its own P + L scale)
     J = torch.zeros((max(net.n_photo, 1), ld), dtype=torch.float64, device="cuda")
     d = G.empty(net.n_species, ld)
@@ -150,6 +167,7 @@ def test_equilibrium_matches_oracle_on_gpu(oracle, network, cfg, ncol_max, shift
     kf, kr = oracle.rate_coeffs(net, T, P, np.zeros((net.n_photo, ld)), ncol)
     _, wp, wl = oracle.source(net, kf, kr, got[0], ncol)
     scale = (wp + wl)[:, :ncol]
-    big = np.isfinite(scale) & (scale > 1e-200)
+    big = np.isfinite(scale) & (scale > 1e-200) & ~touched_by_underflow(net, got[0], ncol)
+    assert big.any()
     assert np.all(np.abs(G.host(d)[:, :ncol])[big] <= 1e-7 * scale[big])
     h.close()
