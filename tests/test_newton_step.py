@@ -173,12 +173,13 @@ def test_newton_step_matches_oracle_on_gpu(oracle, network, cfg, stiffness, ncol
 
 @pytest.mark.gpu
 def test_newton_step_several_column_chunks_on_gpu(oracle, network):
-    """2 100 columns = two passes of 2 048 + 52: columns from both passes and the ragged tail against the oracle."""
+    """2 500 columns = two passes of 2 368 + 132 (the call works through the batch in passes of 148 x 16 columns to
+    bound its workspace): columns from both passes and the ragged tail against the oracle."""
     import torch
     assert torch.cuda.is_available()
     from paper_2512_06729_b200 import synth
     net = network(2)
-    atm = synth.make_atmosphere(71, net, 1, 2100)
+    atm = synth.make_atmosphere(71, net, 1, 2500)
     ncol, ld = atm.ncol, atm.ld
     kf, kr = oracle.rate_coeffs(net, atm.T, atm.P, atm.J, ncol)
     n = atm.n
@@ -191,7 +192,7 @@ def test_newton_step_several_column_chunks_on_gpu(oracle, network):
     h.newton_step(ncol, ld, G.dev(kf), G.dev(kr), G.dev(n), G.dev(dt), dy, dd, workspace=ws)
     h.check_status()
     delta, y_new = G.host(dd), G.host(dy)
-    cols = np.array([0, 31, 32, 2047, 2048, 2049, 2079, 2080, 2099])
+    cols = np.array([0, 31, 32, 2367, 2368, 2369, 2399, 2400, 2499])
     sub = lambda a: np.ascontiguousarray(a[..., cols])
     compare(oracle, net, sub(kf), sub(kr), sub(n), sub(dt), sub(y), cols.size, sub(delta), sub(y_new), "xod_newton_step over column chunks")
     assert np.all(np.isfinite(delta[:, :ncol])) and np.all(np.isnan(delta[:, ncol:]))
