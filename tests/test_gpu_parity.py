@@ -380,8 +380,9 @@ def test_full_size_config4_whole_batch(xod, oracle, network):
     G.check_sum(got_pl, want, scale, cols, "full-size fused dn/dt (P/L variant)")
     G.check_sum(gp, wp, scale, cols, "full-size fused P")
     G.check_sum(gl, wl, scale, cols, "full-size fused L")
-    # excluded columns: NaN only where the oracle has NaN (an overflowed k_r met a zero density)
-    assert np.array_equal(np.isnan(got[:, c]).any(axis=0), np.isnan(want[:, c]).any(axis=0))
+    # excluded columns: wherever the oracle's value left the double range (an overflowed k_r), the GPU's did too; the
+    # GPU may have more such entries, because a partial product of k n n n can overflow first (reading R5, second part)
+    assert not np.isfinite(got[:, c][~np.isfinite(want[:, c])]).any()
 
 
 def test_full_size_config5_jacobian_whole_atmospheres(xod, oracle, network):
