@@ -253,15 +253,15 @@ def stage_timings(binding, h3, net, dev, ws_for, dfma_per_s):
     nr, ns = net.n_reactions, net.n_species
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")        # > 126 MB L2
 
-    best = [None]
+    best_run = [None]      # best of the repeated runs of the last timed() call
 
     def timed(fn, reps, flush_l2):
-        best[0] = None
+        best_run[0] = None
         for _ in range(3):
             fn()
         if not flush_l2:     # SURVEY 8(d) timing protocol: back-to-back calls between two events, repeated; median (and best)
             runs = sorted(event_time_ms(fn, reps, sync) for _ in range(5))
-            best[0] = runs[0]
+            best_run[0] = runs[0]
             return runs[len(runs) // 2]
         tot = 0.0
         for _ in range(reps):
@@ -311,8 +311,8 @@ def stage_timings(binding, h3, net, dev, ws_for, dfma_per_s):
         for name, fn in calls.items():
             ms = timed(fn, reps, big)
             res[name + "_ms"] = ms
-            if best[0] is not None:
-                res[name + "_best_ms"] = best[0]
+            if best_run[0] is not None:
+                res[name + "_best_ms"] = best_run[0]
             if name in ("rate_coeffs", "source", "source_fused"):
                 res[name + "_evals_per_s"] = ncol * nr / (ms * 1e-3)
         if not big:
