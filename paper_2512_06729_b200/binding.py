@@ -129,8 +129,8 @@ class Network:
          self.n_jac_terms) = [x.value for x in v]
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().xod_network_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:     # at interpreter exit the module globals may be gone already
+            _lib.xod_network_destroy(self._h)
             self._h = None
 
     __del__ = close
