@@ -314,8 +314,8 @@ class Photo:
         self.n_bins = d.n_bins
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().xod_photo_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.xod_photo_destroy(self._h)
             self._h = None
 
     __del__ = close
